@@ -1,0 +1,492 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (no GPU).
+
+north_star checks: (1) analytic point-source fluence, (2) infinite-medium closed form, (3) particle
+balance, (4) quadrature integrates harmonics, (5) mirror symmetry, (6) brute force on 4^3.
+Plus closed forms of SURVEY.md 8(c) "What pins each part". None of the expected values below comes
+from the oracle or from the CUDA path.
+"""
+import math
+
+import numpy as np
+import pytest
+from numpy.polynomial import legendre as npleg
+
+from paper_1811_12391_b200.inputs import make_problem, quadrature
+
+pytestmark = pytest.mark.filterwarnings("ignore")
+
+
+def _mesh(nx, ny, nz, dx, dy=None, dz=None):
+    dy = dx if dy is None else dy
+    dz = dx if dz is None else dz
+    return {"nx": nx, "ny": ny, "nz": nz, "dx": dx, "dy": dy, "dz": dz,
+            "x0": -0.5 * nx * dx, "y0": -0.5 * ny * dy, "z0": -0.5 * nz * dz}
+
+
+def _iso_source(pos):
+    return {"pos": tuple(pos), "axis": (0.0, 0.0, -1.0), "up": (0.0, 1.0, 0.0), "tan_half_fan": 0.0,
+            "tan_half_cone": 0.0, "isotropic": 1}
+
+
+def _centres(mesh):
+    x = mesh["x0"] + (np.arange(mesh["nx"]) + 0.5) * mesh["dx"]
+    y = mesh["y0"] + (np.arange(mesh["ny"]) + 0.5) * mesh["dy"]
+    z = mesh["z0"] + (np.arange(mesh["nz"]) + 0.5) * mesh["dz"]
+    return np.meshgrid(z, y, x, indexing="ij")  # each [nz][ny][nx]
+
+
+def _legendre_p(l, x):
+    c = np.zeros(l + 1)
+    c[l] = 1.0
+    return npleg.legval(x, c)
+
+
+# ------------------------------------------------------------------ (4) quadrature + harmonics ---
+@pytest.mark.parametrize("sn,L", [(2, 0), (4, 1), (6, 2), (8, 3), (12, 4), (16, 5)])
+def test_quadrature_integrates_harmonics(orc, sn, L):
+    """PAPER.md:45 N(N+2) directions; sum w = 1; sum_n w Y_lm Y_l'm' = delta/(2l+1) for 2L <= N."""
+    q = quadrature.level_symmetric(sn)
+    n_ang = len(q["w"])
+    assert n_ang == sn * (sn + 2)
+    assert abs(q["w"].sum() - 1.0) < 1e-14
+    assert np.allclose(q["mu"] ** 2 + q["eta"] ** 2 + q["xi"] ** 2, 1.0, atol=1e-13)
+    Y = np.array([orc.harmonics(q["mu"][n], q["eta"][n], q["xi"][n], L) for n in range(n_ang)])
+    gram = (Y * q["w"][:, None]).T @ Y
+    expect = np.diag([1.0 / (2 * l + 1) for l in range(L + 1) for _ in range(2 * l + 1)])
+    assert np.abs(gram - expect).max() < 1e-12
+
+
+def test_quadrature_octant_order():
+    """bit0 <=> mu<0, bit1 <=> eta<0, bit2 <=> xi<0; octant-major ordering."""
+    q = quadrature.level_symmetric(8)
+    per = len(q["w"]) // 8
+    for o in range(8):
+        s = slice(o * per, (o + 1) * per)
+        assert np.all((q["mu"][s] < 0) == bool(o & 1))
+        assert np.all((q["eta"][s] < 0) == bool(o & 2))
+        assert np.all((q["xi"][s] < 0) == bool(o & 4))
+
+
+def test_harmonics_low_orders_explicit(orc):
+    """P1 moments are (1, eta, xi, mu) in index order 0..3; l=2 against the textbook real forms."""
+    mu, eta = 0.3, -0.5
+    xi = math.sqrt(1 - mu * mu - eta * eta)
+    y = orc.harmonics(mu, eta, xi, 2)
+    s3 = math.sqrt(3.0)
+    expect = [1.0, eta, xi, mu,
+              s3 * mu * eta,                 # l=2, m=-2: sqrt(3)/2 sin^2 sin(2phi) = sqrt(3) mu eta
+              s3 * eta * xi,                 # m=-1
+              0.5 * (3 * xi * xi - 1),       # m=0
+              s3 * mu * xi,                  # m=+1
+              0.5 * s3 * (mu * mu - eta * eta)]
+    assert np.allclose(y, expect, atol=1e-14)
+
+
+def test_addition_theorem(orc):
+    """sum_m Y_lm(a) Y_lm(b) = P_l(a.b) for l <= 5 (random directions, and the poles)."""
+    rng = np.random.default_rng(7)
+    v = rng.normal(size=(12, 3))
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    v[0] = (0, 0, 1.0)
+    v[1] = (0, 0, -1.0)
+    for a in v:
+        for b in v:
+            ya, yb = orc.harmonics(*a, 5), orc.harmonics(*b, 5)
+            for l in range(6):
+                s = sum(ya[l * (l + 1) + m] * yb[l * (l + 1) + m] for m in range(-l, l + 1))
+                assert abs(s - _legendre_p(l, float(a @ b))) < 1e-13
+
+
+# ------------------------------------------------------------------ (1) ray trace -----------------
+def _slab_length(mesh, s, c):
+    """Length of the segment s->c inside the box, by the ray-box slab formula."""
+    s, c = np.asarray(s, float), np.asarray(c, float)
+    d = c - s
+    lo = np.array([mesh["x0"], mesh["y0"], mesh["z0"]])
+    hi = lo + np.array([mesh["nx"] * mesh["dx"], mesh["ny"] * mesh["dy"], mesh["nz"] * mesh["dz"]])
+    t0, t1 = 0.0, 1.0
+    for a in range(3):
+        ta, tb = (lo[a] - s[a]) / d[a], (hi[a] - s[a]) / d[a]
+        t0, t1 = max(t0, min(ta, tb)), min(t1, max(ta, tb))
+    return max(t1 - t0, 0.0) * np.linalg.norm(d)
+
+
+def test_uncollided_pure_absorber_analytic(orc):
+    """north_star check 1: homogeneous pure absorber, phi_u = S exp(-sigma_t l_box) / (4 pi r^2)."""
+    mesh = _mesh(7, 6, 5, 1.3, 0.9, 1.1)
+    mat = np.zeros((5, 6, 7), np.uint8)
+    sig_t = np.array([[0.21, 0.47]])
+    spec = np.array([0.3, 0.7])
+    pos = (30 * 2 / 7, -30 * 3 / 7, 30 * 6 / 7)
+    phi, path = orc.uncollided(mesh, mat, sig_t, _iso_source(pos), spec, want_path=True)
+    Z, Y, X = _centres(mesh)
+    for k in range(5):
+        for j in range(6):
+            for i in range(7):
+                c = (X[k, j, i], Y[k, j, i], Z[k, j, i])
+                ell = _slab_length(mesh, pos, c)
+                r2 = sum((a - b) ** 2 for a, b in zip(c, pos))
+                assert abs(path[k, j, i] - ell) < 1e-12          # telescoping sum of segments
+                for g in range(2):
+                    ex = spec[g] * math.exp(-sig_t[0, g] * ell) / (4 * math.pi * r2)
+                    assert abs(phi[g, k, j, i] - ex) <= 1e-13 * ex
+
+
+def test_uncollided_void_is_inverse_square(orc):
+    mesh = _mesh(5, 5, 5, 2.0)
+    mat = np.zeros((5, 5, 5), np.uint8)
+    pos = (1.234, -20.0, 3.21)
+    phi = orc.uncollided(mesh, mat, np.zeros((1, 3)), _iso_source(pos), np.array([0.2, 0.3, 0.5]))
+    Z, Y, X = _centres(mesh)
+    r2 = (X - pos[0]) ** 2 + (Y - pos[1]) ** 2 + (Z - pos[2]) ** 2
+    for g, s in enumerate([0.2, 0.3, 0.5]):
+        assert np.allclose(phi[g] * 4 * math.pi * r2, s, rtol=1e-14)
+
+
+def _dda_tau(mesh, mat, sig, s, c):
+    """Independent exact method: incremental (Amanatides-Woo) stepping from s to c."""
+    s, c = np.asarray(s, float), np.asarray(c, float)
+    d = c - s
+    r = np.linalg.norm(d)
+    n = np.array([mesh["nx"], mesh["ny"], mesh["nz"]])
+    h = np.array([mesh["dx"], mesh["dy"], mesh["dz"]])
+    o = np.array([mesh["x0"], mesh["y0"], mesh["z0"]])
+    t0, t1 = 0.0, 1.0
+    for a in range(3):
+        if d[a] == 0:
+            continue
+        ta, tb = (o[a] - s[a]) / d[a], (o[a] + n[a] * h[a] - s[a]) / d[a]
+        t0, t1 = max(t0, min(ta, tb)), min(t1, max(ta, tb))
+    if t1 <= t0:
+        return 0.0
+    p = s + (t0 + 1e-12) * d
+    idx = np.clip(np.floor((p - o) / h).astype(int), 0, n - 1)
+    step = np.where(d > 0, 1, -1)
+    tmax = np.full(3, np.inf)
+    for a in range(3):
+        if d[a] != 0:
+            plane = o[a] + (idx[a] + (1 if d[a] > 0 else 0)) * h[a]
+            tmax[a] = (plane - s[a]) / d[a]
+    t, tau = t0, 0.0
+    while t < t1 - 1e-15:
+        a = int(np.argmin(tmax))
+        tn = min(tmax[a], t1)
+        tau += sig[mat[idx[2], idx[1], idx[0]]] * (tn - t) * r
+        t = tn
+        idx[a] += step[a]
+        if idx[a] < 0 or idx[a] >= n[a]:
+            break
+        plane = o[a] + (idx[a] + (1 if d[a] > 0 else 0)) * h[a]
+        tmax[a] = (plane - s[a]) / d[a]
+    return tau
+
+
+def test_uncollided_heterogeneous_vs_dda_and_midpoint(orc):
+    """Heterogeneous medium: sorted-alpha list (oracle) vs incremental DDA (1e-12) and vs
+    midpoint-rule sampling of sigma_t along the ray (1e-4)."""
+    rng = np.random.default_rng(11)
+    mesh = _mesh(8, 6, 5, 0.7, 0.9, 1.1)
+    mat = rng.integers(0, 3, size=(5, 6, 8)).astype(np.uint8)
+    sig = np.array([[0.02], [0.35], [0.9]])
+    pos = (7.3, -11.1, 4.9)
+    phi = orc.uncollided(mesh, mat, sig, _iso_source(pos), np.array([1.0]))[0]
+    Z, Y, X = _centres(mesh)
+    o = np.array([mesh["x0"], mesh["y0"], mesh["z0"]])
+    h = np.array([mesh["dx"], mesh["dy"], mesh["dz"]])
+    n = np.array([8, 6, 5])
+    for (k, j, i) in [(0, 0, 0), (4, 5, 7), (2, 3, 4), (1, 5, 0), (3, 0, 6), (4, 2, 2), (0, 4, 7)]:
+        c = np.array([X[k, j, i], Y[k, j, i], Z[k, j, i]])
+        r2 = ((c - pos) ** 2).sum()
+        tau_o = -math.log(phi[k, j, i] * 4 * math.pi * r2)
+        assert abs(tau_o - _dda_tau(mesh, mat, sig[:, 0], pos, c)) < 1e-12
+        ns = 200000
+        t = (np.arange(ns) + 0.5) / ns
+        pts = np.asarray(pos)[None, :] + t[:, None] * (c - pos)[None, :]
+        q = np.floor((pts - o) / h).astype(int)
+        ok = np.all((q >= 0) & (q < n), axis=1)
+        q = np.clip(q, 0, n - 1)
+        tau_m = (sig[mat[q[:, 2], q[:, 1], q[:, 0]], 0] * ok).sum() / ns * math.sqrt(r2)
+        assert abs(tau_o - tau_m) < 1e-4 * max(tau_m, 1.0)
+
+
+def test_uncollided_collimation_and_sn_independence(orc):
+    """Reading R8: rectangular pyramid, boundary inclusive, exact zeros outside;
+    phi_u does not depend on S_N or P_L."""
+    p = make_problem("config2", nx=16, ny=16, nz=8, voxel=2.4, n_group=3, sn=4, pl=1)
+    src = p["sources"][0]
+    phi = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+    Z, Y, X = _centres(p["mesh"])
+    a = 54.0 - Y                      # d . axis with axis (0,-1,0), source at (0,54,0)
+    inside = (np.abs(Z) <= a * src["tan_half_cone"]) & (np.abs(X) <= a * src["tan_half_fan"])
+    assert inside.any() and (~inside).any()
+    assert np.all(phi[:, ~inside] == 0.0)
+    assert np.all(phi[:, inside] > 0.0)
+    p2 = make_problem("config2", nx=16, ny=16, nz=8, voxel=2.4, n_group=3, sn=8, pl=3)
+    phi2 = orc.uncollided(p2["mesh"], p2["material"], p2["sigma_t"], p2["sources"][0], p2["spectrum"])
+    assert np.array_equal(phi, phi2)
+
+
+# ------------------------------------------------------------------ DD cell closed forms ----------
+def test_single_cell_closed_form(orc):
+    """1x1x1 mesh, isotropic Q, vacuum: phi = Q sum_n w_n / (sigma_t + cx + cy + cz)."""
+    q = quadrature.level_symmetric(6)
+    mesh = _mesh(1, 1, 1, 0.8, 1.1, 1.7)
+    sig_t, Q0 = 0.37, 2.5
+    Q = np.zeros((4, 1, 1, 1))
+    Q[0] = Q0
+    phi = orc.sweep(mesh, np.zeros((1, 1, 1), np.uint8), [sig_t], q, 1, Q)
+    den = sig_t + 2 * np.abs(q["mu"]) / 0.8 + 2 * np.abs(q["eta"]) / 1.1 + 2 * np.abs(q["xi"]) / 1.7
+    assert abs(phi[0, 0, 0, 0] - Q0 * (q["w"] / den).sum()) < 1e-14
+    # first-moment rows: sum w Omega psi vanishes by symmetry for an isotropic source in one cell
+    assert np.abs(phi[1:, 0, 0, 0]).max() < 1e-15
+
+
+def test_one_d_diamond_factor_and_fixup(orc):
+    """n x 1 x 1 pure absorber, source only in the first cell, wide transverse cells (vacuum transverse
+    inflow): with s = sigma_t + c_y + c_z each ordinate obeys psi_out/psi_in = (c_x - s)/(c_x + s), the
+    textbook 1-D diamond factor (2|mu| - s dx)/(2|mu| + s dx), while positive; once s > c_x the
+    set-to-zero fixup pins psi_out = 0 and the balance (c_x/2)(0 - psi_in) + s psi_c = 0 fixes psi_c."""
+    q = quadrature.level_symmetric(2)          # one |mu| = 1/sqrt(3)
+    mu = 1 / math.sqrt(3.0)
+    n = 6
+    for sig_t in (0.2, 3.0):                   # thin: no fixup; thick: fixup after the first cell
+        dx = 1.0
+        mesh = _mesh(n, 1, 1, dx, 1e3, 1e3)
+        Q = np.zeros((1, 1, 1, n))
+        Q[0, 0, 0, 0] = 1.0
+        _, psi = orc.sweep(mesh, np.zeros((1, 1, n), np.uint8), [sig_t], q, 0, Q, want_psi=True)
+        a = next(i for i in range(8) if q["mu"][i] > 0 and q["eta"][i] > 0 and q["xi"][i] > 0)
+        c = 2 * mu / dx
+        s_t = sig_t + 2 * (2 * mu / 1e3)
+        # hand recursion
+        pin, expect = 0.0, []
+        for i in range(n):
+            src = 1.0 if i == 0 else 0.0
+            pc = (src + c * pin) / (s_t + c)
+            pout = 2 * pc - pin
+            if pout < 0:
+                pc = (src + 0.5 * c * pin) / s_t
+                pout = 0.0
+            expect.append(pc)
+            pin = pout
+        assert np.allclose(psi[a], expect, rtol=1e-13, atol=1e-300)
+        if sig_t == 0.2:
+            fac = (2 * mu - s_t * dx) / (2 * mu + s_t * dx)
+            ratios = psi[a][2:] / psi[a][1:-1]
+            assert np.allclose(ratios, fac, rtol=1e-12)
+        else:
+            assert psi[a][1] > 0 and np.all(psi[a][2:] == 0.0)       # outflow pinned to zero
+
+
+# ------------------------------------------------------------------ (3) balance -------------------
+def test_per_sweep_balance_with_fixup(orc):
+    """sum V Q00 = sum V sigma_t phi00 + leakage after ONE sweep, fixup active (thick random medium)."""
+    rng = np.random.default_rng(5)
+    mesh = _mesh(6, 5, 4, 1.0, 1.2, 0.8)
+    mat = rng.integers(0, 3, size=(4, 5, 6)).astype(np.uint8)
+    sig = np.array([0.05, 1.5, 6.0])
+    q = quadrature.level_symmetric(4)
+    Q = np.zeros((4, 4, 5, 6))
+    Q[0] = rng.uniform(0, 1, size=(4, 5, 6)) * (rng.uniform(size=(4, 5, 6)) < 0.3)
+    Q[1:] = 0.2 * rng.normal(size=(3, 4, 5, 6)) * Q[0]
+    phi, leak, psi = orc.sweep(mesh, mat, sig, q, 1, Q, want_leakage=True, want_psi=True)
+    V = 1.0 * 1.2 * 0.8
+    lhs = V * Q[0].sum()
+    rhs = V * (sig[mat] * phi[0]).sum() + leak
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    assert leak > 0
+
+
+def test_converged_balance_and_infinite_medium(orc):
+    """north_star check 3 (source = absorption + leakage, 1e-9, at convergence) on config-1-like water,
+    and check 2 (reflective box, uniform Q: phi = Q/(sigma_t - sigma_s0))."""
+    p = make_problem("config1", nx=6, ny=6, nz=6, n_iter=60)
+    src = p["sources"][0]
+    pu = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+    # the balance identity needs sum_n w_n Y_lm = delta_l0 exactly, so this pin uses the fp64 quadrature
+    # table (the fp32-rounded table every config feeds to both sides breaks it at the 4e-8 level)
+    pc, leak, _ = orc.solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], quadrature.level_symmetric(4), 1, 60,
+                            source_pos=src["pos"], phi_u=pu, want_balance=True)
+    sig_t = p["sigma_t"].astype(float)
+    sig_s0 = p["sigma_s"][:, 0].astype(float)           # [mat][from][to]
+    V = p["mesh"]["dx"] ** 3
+    G = p["n_group"]
+    for g in range(G):
+        # source of collided photons in g: scattering of uncollided (all g' <= g) and of collided g' < g
+        s = sum(sig_s0[0, gp, g] * pu[gp].sum() for gp in range(g + 1))
+        s += sum(sig_s0[0, gp, g] * pc[gp, 0].sum() for gp in range(g))
+        removal = (sig_t[0, g] - sig_s0[0, g, g]) * pc[g, 0].sum()
+        assert abs(V * s - V * removal - leak[g]) < 1e-9 * V * s
+
+    mesh = _mesh(4, 4, 4, 1.0)
+    mat = np.zeros((4, 4, 4), np.uint8)
+    sig_t2 = np.array([[1.0, 1.4]])
+    sig_s = np.zeros((1, 2, 2, 2))
+    sig_s[0, 0] = [[0.5, 0.3], [0.0, 0.6]]
+    sig_s[0, 1] = [[0.2, 0.1], [0.0, 0.25]]
+    qext = np.zeros((2, 4, 4, 4, 4))
+    qext[0, 0], qext[1, 0] = 2.0, 0.7
+    quad = quadrature.level_symmetric(4)
+    phi = orc.solve(mesh, mat, sig_t2, sig_s, quad, 1, 400, q_ext=qext, reflective=True)
+    phi1 = 2.0 / (1.0 - 0.5)
+    phi2 = (0.7 + 0.3 * phi1) / (1.4 - 0.6)              # two-group cascade closed form
+    assert np.allclose(phi[0, 0], phi1, rtol=1e-12)
+    assert np.allclose(phi[1, 0], phi2, rtol=1e-12)
+    assert np.abs(phi[:, 1:]).max() < 1e-12              # no net current in an infinite medium
+
+
+def test_no_ingroup_scatter_iteration_count_irrelevant(orc):
+    """With sigma_s^{g->g} = 0 one iteration equals any number (pins the n_iter convention R5)."""
+    p = make_problem("config1", nx=5, ny=4, nz=3)
+    ss = p["sigma_s"].astype(float).copy()
+    for g in range(p["n_group"]):
+        ss[:, :, g, g] = 0.0
+    src = p["sources"][0]
+    pu = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+    a = orc.solve(p["mesh"], p["material"], p["sigma_t"], ss, p["quadrature"], 1, 1, source_pos=src["pos"], phi_u=pu)
+    b = orc.solve(p["mesh"], p["material"], p["sigma_t"], ss, p["quadrature"], 1, 7, source_pos=src["pos"], phi_u=pu)
+    assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ (5) mirror symmetry -----------
+def test_cylinder_mirror_symmetry(orc):
+    """north_star check 5: x -> -x and z -> -z mirror symmetry of the cylinder result (source on the y axis)."""
+    p = make_problem("config2", nx=12, ny=12, nz=6, voxel=3.2, n_group=3, sn=4, pl=1, n_iter=4)
+    r = orc.run_problem(p)
+    for key in ("phi_u", "phi_c", "dose"):
+        a = r[key]
+        scale = np.abs(a).max()
+        assert np.abs(a - a[..., ::-1]).max() < 1e-12 * scale          # x mirror
+        assert np.abs(a - np.flip(a, axis=-3)).max() < 1e-12 * scale   # z mirror
+    assert np.abs(r["dose"] - r["dose"][:, ::-1, :]).max() > 1e-3 * r["dose"].max()   # y is NOT symmetric
+
+
+# ------------------------------------------------------------------ (6) brute force 4^3 -----------
+def test_brute_force_linear_system_4cubed(orc):
+    """north_star check 6: full linear system (cell-centre + face unknowns, DD closures, zero inflow,
+    direct angle-to-angle P_l kernel of eq. 2) solved by sparse LU vs source iteration run to 1e-13."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+    n = 4
+    mesh = _mesh(n, n, n, 0.9, 1.0, 1.1)
+    h = (0.9, 1.0, 1.1)
+    rng = np.random.default_rng(3)
+    mat = rng.integers(0, 2, size=(n, n, n)).astype(np.uint8)
+    sig_t = np.array([0.20, 0.35])
+    sig_sl = np.array([[0.10, 0.04], [0.20, 0.08]])       # [mat][l], P1
+    quad = quadrature.level_symmetric(4)
+    na = 24
+    Om = np.stack([quad["mu"], quad["eta"], quad["xi"]], axis=1)
+    w = quad["w"]
+    cosm = Om @ Om.T
+    Qiso = rng.uniform(0.9, 1.1, size=(n, n, n))          # isotropic external source, q_n = Q00
+    nv = n ** 3
+    nfx = (n + 1) * n * n
+
+    def cid(i, j, k): return (k * n + j) * n + i
+    def fx(i, j, k): return (k * n + j) * (n + 1) + i     # face at lower x side of cell i
+    def fy(i, j, k): return (k * (n + 1) + j) * n + i
+    def fz(i, j, k): return (k * n + j) * n + i
+    per = nv + 3 * nfx
+    rows, cols, vals, rhs = [], [], [], []
+    def add(r, c, v): rows.append(r); cols.append(c); vals.append(v)
+    r = 0
+    for a in range(na):
+        base = a * per
+        off = (base + nv, base + nv + nfx, base + nv + 2 * nfx)
+        for k in range(n):
+            for j in range(n):
+                for i in range(n):
+                    c = cid(i, j, k)
+                    m = mat[k, j, i]
+                    lo = (off[0] + fx(i, j, k), off[1] + fy(i, j, k), off[2] + fz(i, j, k))
+                    hi = (off[0] + fx(i + 1, j, k), off[1] + fy(i, j + 1, k), off[2] + fz(i, j, k + 1))
+                    # balance: sum_d Omega_d/h_d (psi_hi - psi_lo) + sigma_t psi_c - scatter = q
+                    for d in range(3):
+                        add(r, hi[d], Om[a, d] / h[d]); add(r, lo[d], -Om[a, d] / h[d])
+                    add(r, base + c, sig_t[m])
+                    for b in range(na):
+                        kern = w[b] * sum((2 * l + 1) * sig_sl[m, l] * _legendre_p(l, cosm[a, b]) for l in range(2))
+                        add(r, b * per + c, -kern)
+                    rhs.append(Qiso[k, j, i]); r += 1
+                    for d in range(3):                    # diamond closures
+                        add(r, base + c, 1.0); add(r, lo[d], -0.5); add(r, hi[d], -0.5)
+                        rhs.append(0.0); r += 1
+        for k in range(n):                                # vacuum inflow
+            for j in range(n):
+                add(r, off[0] + fx(0 if Om[a, 0] > 0 else n, j, k), 1.0); rhs.append(0.0); r += 1
+        for k in range(n):
+            for i in range(n):
+                add(r, off[1] + fy(i, 0 if Om[a, 1] > 0 else n, k), 1.0); rhs.append(0.0); r += 1
+        for j in range(n):
+            for i in range(n):
+                add(r, off[2] + fz(i, j, 0 if Om[a, 2] > 0 else n), 1.0); rhs.append(0.0); r += 1
+    assert r == na * per
+    A = sp.csc_matrix((vals, (rows, cols)), shape=(r, r))
+    sol = spla.spsolve(A, np.array(rhs))
+    psi = np.array([sol[a * per:a * per + nv] for a in range(na)])
+    faces = np.concatenate([sol[a * per + nv:(a + 1) * per] for a in range(na)])
+    assert psi.min() > 0 and faces.min() > -1e-14          # fixup inactive, so SI solves the same system
+    bf = [(w[:, None] * psi).sum(0)] + [(w[:, None] * Om[:, d:d + 1] * psi).sum(0) for d in (1, 2, 0)]
+
+    sig_t_tab = sig_t[:, None]
+    sig_s = np.zeros((2, 2, 1, 1))
+    sig_s[:, :, 0, 0] = sig_sl
+    qext = np.zeros((1, 4, n, n, n))
+    qext[0, 0] = Qiso
+    phi = orc.solve(mesh, mat, sig_t_tab, sig_s, quad, 1, 200, q_ext=qext)
+    for lm in range(4):                                    # (phi, sum w eta psi, sum w xi psi, sum w mu psi)
+        assert np.abs(phi[0, lm].ravel() - bf[lm]).max() < 1e-12 * np.abs(bf[0]).max()
+
+
+def test_moment_scatter_equals_direct_angle_sum(orc):
+    """Reading R2: the moment form of the scattering source equals the direct double sum
+    sum_n' w_n' sum_l (2l+1) sigma_sl P_l(Omega_n.Omega_n') psi_n' (P3, S8), using stored angular flux."""
+    rng = np.random.default_rng(9)
+    quad = quadrature.level_symmetric(8)
+    L = 3
+    mesh = _mesh(3, 3, 3, 1.0)
+    mat = np.zeros((3, 3, 3), np.uint8)
+    Q = np.zeros((16, 3, 3, 3))
+    Q[0] = rng.uniform(0.5, 1.0, size=(3, 3, 3))
+    phi, psi = orc.sweep(mesh, mat, [0.4], quad, L, Q, want_psi=True)
+    sig_sl = np.array([0.3, 0.12, 0.05, 0.02])
+    Om = np.stack([quad["mu"], quad["eta"], quad["xi"]], axis=1)
+    cosm = np.clip(Om @ Om.T, -1, 1)
+    kern = sum((2 * l + 1) * sig_sl[l] * _legendre_p(l, cosm) for l in range(L + 1)) * quad["w"][None, :]
+    direct = kern @ psi                                     # [n][cell]
+    Qs = np.zeros_like(Q)
+    for l in range(L + 1):
+        for m in range(-l, l + 1):
+            Qs[l * (l + 1) + m] = sig_sl[l] * phi[l * (l + 1) + m]
+    # moment-to-discrete of Qs, written out with the oracle's harmonics only as the basis functions
+    for nidx in (0, 17, 45, 79):
+        y = orc.harmonics(*Om[nidx], L)
+        qn = sum((2 * l + 1) * y[l * (l + 1) + m] * Qs[l * (l + 1) + m] for l in range(L + 1) for m in range(-l, l + 1))
+        assert np.abs(qn.ravel() - direct[nidx]).max() < 1e-13
+
+
+# ------------------------------------------------------------------ dose --------------------------
+def test_dose_linear_functional_and_air_zero(orc):
+    """D = sum_g K[mat][g] (phi_u + phi_c00); air row of K = 0 => D = 0 in air."""
+    mesh = _mesh(2, 1, 1, 1.0)
+    mat = np.array([[[0, 1]]], np.uint8)
+    K = np.array([[0.0, 0.0], [2.0, 3.0]])
+    pu = np.array([[[[1.0, 10.0]]], [[[2.0, 20.0]]]])
+    pc = np.zeros((2, 4, 1, 1, 2))
+    pc[0, 0, 0, 0] = [0.5, 5.0]
+    pc[1, 0, 0, 0] = [0.25, 2.5]
+    pc[:, 1:] = 99.0                                       # higher moments must not enter
+    tot, d = orc.dose(mesh, mat, K, pu, pc)
+    assert np.array_equal(tot[:, 0, 0, 1], [15.0, 22.5])
+    assert d[0, 0, 0] == 0.0 and d[0, 0, 1] == 2.0 * 15.0 + 3.0 * 22.5
+    _, d2 = orc.dose(mesh, mat, K, pu, pc, dose_in=d)
+    assert np.array_equal(d2, 2 * d)
+
+
+def test_water_mean_free_path():
+    """photon mean free path in water 13.9 mm at 20 keV (calibration of the synthetic xs)."""
+    from paper_1811_12391_b200.inputs import xs
+    mu20 = xs.mu_pe("water", 20.0) + 3.343e23 * 2 * math.pi * np.sum(
+        xs.kn_dsigma_domega(20.0, xs._XM)[0] * xs._WM)
+    assert abs(10.0 / mu20 - 13.9) < 0.05
