@@ -1,0 +1,161 @@
+/* dos.h -- C ABI of the discrete-ordinates CT dose hot path on one B200 (sm_100a).
+ *
+ * Method: Norris & Liu, "Photon Fluence and Dose Estimation in CT using a Discrete Ordinates
+ * Boltzmann Solver", arXiv 1811.12391 (text: /root/reference/PAPER.md; cited below as PAPER.md:line).
+ * Readings of points the paper leaves open are R1..R18 in DESIGN.md.
+ *
+ * Conventions
+ *   - "host" pointers are ordinary CPU memory and are COPIED during the call that takes them.
+ *   - "device" pointers (prefix d_) are CUDA device memory owned by the caller (e.g. torch tensors).
+ *     The library never allocates device memory: all of its state lives in the caller's workspace,
+ *     which must stay alive and untouched until dos_destroy.
+ *   - Every call only ENQUEUES work on the CUDA stream given to dos_create (no host sync), except
+ *     the *_host entry points, which synchronise that stream before returning.
+ *   - Fields are [..][nz][ny][nx], x fastest. Group index 0 is the HIGHEST energy.
+ *   - Errors: a negative dos_status, never an exception; text via dos_last_error().
+ *   - Call order: dos_create -> dos_uncollided -> dos_solve -> dos_fluence / dos_dose (any order,
+ *     any number of times) -> dos_uncollided (next source position) ...; out-of-order = DOS_ERR_STATE.
+ */
+#ifndef DOS_H_
+#define DOS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dos_ctx dos_ctx; /* opaque; created by dos_create, freed by dos_destroy */
+
+typedef enum {
+    DOS_OK = 0,
+    DOS_ERR_INVALID_ARG = -1, /* null pointer, non-positive size, bad table values            */
+    DOS_ERR_SHAPE = -2,       /* sizes inconsistent with each other / workspace too small     */
+    DOS_ERR_STATE = -3,       /* call out of order                                            */
+    DOS_ERR_NOMEM = -4,       /* host allocation failed                                       */
+    DOS_ERR_CUDA = -5,        /* a CUDA runtime call or an earlier kernel failed              */
+    DOS_ERR_UNSUPPORTED = -6  /* valid request outside what this build implements             */
+} dos_status;
+
+/* 3-D Cartesian voxel mesh. (x0,y0,z0) = lower corner in cm; voxel (i,j,k) has its
+ * centre at x0 + (i + 1/2) dx, ... */
+typedef struct {
+    int32_t nx, ny, nz;
+    double dx, dy, dz;
+    double x0, y0, z0;
+} dos_mesh;
+
+/* Multigroup macroscopic cross sections per material id and dose factors
+ * (PAPER.md:47, :93). All host, all fp32.
+ *   sigma_t [n_mat][G]                    1/cm, > 0
+ *   sigma_s [n_mat][n_leg+1][G from][G to] Legendre moments sigma_sl^{g'->g}; entries with to < from
+ *                                         (upscatter) must be 0: eq. 2's g' sum is one-sided
+ *                                         (reading R1)
+ *   kerma   [n_mat][G]                    dose per unit fluence; a zero row neglects dose in that
+ *                                         material (air)                        */
+typedef struct {
+    int32_t n_mat, n_group, n_leg;
+    const float *sigma_t;
+    const float *sigma_s;
+    const float *kerma;
+} dos_xs;
+
+/* S_N quadrature (PAPER.md:43-45 eq. 3, :79). Host fp32 arrays of length n_ang = 8 * per_octant,
+ * octant-major: octant o = bit0 (mu<0) | bit1 (eta<0) | bit2 (xi<0) holds entries
+ * [o*per_octant, (o+1)*per_octant), and entry t of octant o is the mirror image of entry t of
+ * octant 0 with the same weight. sum(w) = 1 (reading R4). */
+typedef struct {
+    int32_t n_ang;
+    const float *mu, *eta, *xi, *w;
+} dos_quadrature;
+
+/* Point source with rectangular-pyramid collimation ("position ... two additional
+ * parameters phi and theta"; reading R8). axis, up: unit vectors, up perpendicular to axis. A voxel
+ * centre c is inside the beam iff isotropic != 0, or with d = c - pos, a = d.axis > 0:
+ * |d.up| <= a tan_half_cone and |d.(axis x up)| <= a tan_half_fan (boundary inclusive). */
+typedef struct {
+    double pos[3];
+    double axis[3];
+    double up[3];
+    double tan_half_fan, tan_half_cone;
+    int32_t isotropic;
+} dos_source;
+
+/* Bytes of device workspace dos_create needs for this problem (n_batch must be 1 in this build). */
+dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs, const dos_quadrature *quad,
+                               int32_t P_L, int32_t n_batch, size_t *bytes_out);
+
+/* Build a context: validates and copies the host tables, precomputes the moment-to-discrete and
+ * discrete-to-moment matrices ((2l+1) Y_lm(Omega_n) and w_n Y_lm(Omega_n); real Schmidt
+ * semi-normalised harmonics, (P_L+1)^2 moments; readings R2, R10) and the diamond-difference
+ * constants 2|Omega_d|/Delta_d, and lays out the workspace.
+ *   d_material_ids  device uint8 [nz][ny][nx], values < n_mat (checked on the device at the first
+ *                   dos_uncollided); caller-owned, must outlive the context
+ *   P_L             scattering order used, 0 <= P_L <= min(xs->n_leg, 5)
+ *   d_workspace     device, >= dos_workspace_bytes, 256-byte aligned
+ *   cuda_stream     a cudaStream_t (NULL = legacy default stream)                                  */
+dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint8_t *d_material_ids,
+                      const dos_xs *xs, const dos_quadrature *quad, int32_t P_L, void *d_workspace,
+                      size_t workspace_bytes, void *cuda_stream);
+
+/* Replace the material grid from HOST memory (copied into the workspace; the context then uses that
+ * copy instead of d_material_ids). Used by the end-to-end path. */
+dos_status dos_set_material_host(dos_ctx *ctx, const uint8_t *h_material_ids);
+
+/* Uncollided fluence by ray tracing (readings R6-R9): for every voxel centre inside
+ * the beam, phi_u^g = S_g exp(-sum_cells sigma_t^g l_cell) / (4 pi r^2) with exact (Siddon) segment
+ * lengths from the source to the voxel CENTRE, no attenuation outside the mesh; 0 outside the beam.
+ * Accumulated and exponentiated in fp64, stored as fp32 in the workspace.
+ *   spectrum        host [G], source particles per group (sum = 1 for "per source particle")
+ *   d_phi_u_out     device [G][nz][ny][nx] or NULL: also copy the result there                      */
+dos_status dos_uncollided(dos_ctx *ctx, const dos_source *source, const float *spectrum,
+                          float *d_phi_u_out);
+
+/* Collided fluence (PAPER.md:39-45 eq. 2-3, :49): for g = 0..G-1, top-down (downscatter only):
+ *   Q_fix = first-collision source moments Y_lm(Omega_r) sum_{g'<=g} sigma_sl^{g'->g} phi_u^{g'}
+ *           + sum_{g'<g} sigma_sl^{g'->g} phi_c^{g'}[lm]
+ *   n_iter source iterations from phi = 0: Q = Q_fix + sigma_sl^{g->g} phi; phi = Sweep(Q)
+ * Sweep = all N_a ordinates, diamond difference with set-to-zero fixup and rebalance (north_star;
+ * readings R3, R11, R12), vacuum boundaries, fp32. No convergence test (reading R5). */
+dos_status dos_solve(dos_ctx *ctx, int32_t n_iter);
+
+/* Scalar fluence per group: collided phi_c^g = phi^g[00] and/or total phi_u^g + phi_c^g.
+ * Either pointer may be NULL. device [G][nz][ny][nx] fp32. */
+dos_status dos_fluence(dos_ctx *ctx, float *d_phi_collided, float *d_phi_total);
+
+/* Dose map D(c) = sum_g kerma[m(c)][g] (phi_u^g + phi_c^g)(c). device [nz][ny][nx];
+ * accumulate != 0 adds to what d_dose holds (axial scan: doses of source positions summed). */
+dos_status dos_dose(dos_ctx *ctx, float *d_dose, int32_t accumulate);
+
+/* Same as dos_dose, result copied to HOST memory [nz][ny][nx]; synchronises the stream. With
+ * accumulate != 0 the device-side running sum kept in the workspace is extended and returned. */
+dos_status dos_dose_host(dos_ctx *ctx, float *h_dose, int32_t accumulate);
+
+/* Tuning / measurement knobs (all optional).
+ *   "sweep_chunk"   cells along x between face-flux hand-offs of neighbouring tiles (>= 1)
+ *   "profile"       1: bracket every sweep and ray-trace launch with CUDA events (see dos_profile)  */
+dos_status dos_set_option(dos_ctx *ctx, const char *name, int64_t value);
+
+/* Accumulated device time (ms, CUDA events on the context's stream) and launch counts since the last
+ * dos_profile_reset, for the two named kernels. Synchronises the stream. Needs option profile=1. */
+typedef struct {
+    double sweep_ms;
+    int64_t sweep_launches;
+    double raytrace_ms;
+    int64_t raytrace_launches;
+    int64_t kernel_launches; /* every kernel this library launched, all kinds */
+} dos_profile_t;
+dos_status dos_profile(dos_ctx *ctx, dos_profile_t *out);
+dos_status dos_profile_reset(dos_ctx *ctx);
+
+void dos_destroy(dos_ctx *ctx);
+
+/* Text of the last error of this context ("" if none); with ctx == NULL, of the last failed
+ * dos_create / dos_workspace_bytes in this thread. The pointer stays valid until the next call. */
+const char *dos_last_error(const dos_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DOS_H_ */

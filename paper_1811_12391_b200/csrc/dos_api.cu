@@ -1,0 +1,506 @@
+// dos_api.cu -- the C ABI of include/dos.h: context, validation, workspace layout, host-side tables,
+// and the launch sequence of the hot path. Kernels: dos_kernels.cu (ray trace, sources, dose) and
+// dos_sweep.cu (transport sweep). No code is shared with oracle/.
+#include "../../include/dos.h"
+#include "dos_internal.h"
+#include "dos_kernels.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+struct Layout {
+    size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
+        spectrum, errflag, total;
+};
+
+struct dos_ctx {
+    dos_mesh mesh;
+    int n_mat, G, n_leg, L, M, MP, n_ang, per_oct;
+    int ntj, ntk, n_items, ag, n_grp, chunk, grid;
+    size_t nv;
+    cudaStream_t stream;
+    const uint8_t *d_mat;        // current material grid (caller's or the workspace copy)
+    char *ws;
+    Layout lay;
+    std::vector<int> band_lo;    // [G]: lowest g' with a non-zero sigma_s^{g'->g}
+    int state;                   // 0 created, 1 uncollided done, 2 solved
+    dos_source src;
+    bool have_dose_acc;
+    bool profile;
+    std::vector<cudaEvent_t> ev;  // pairs (start, stop); kind in ev_kind
+    std::vector<int> ev_kind;     // 0 sweep, 1 ray trace
+    double acc_ms[2];
+    int64_t acc_n[2];
+    int64_t launches;
+    std::string err;
+};
+
+static thread_local std::string g_err;
+
+static dos_status fail(dos_ctx *c, dos_status s, const std::string &msg)
+{
+    if (c) c->err = msg; else g_err = msg;
+    return s;
+}
+
+#define CUDA_TRY(c, call)                                                                              \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail((c), DOS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+    } while (0)
+
+// Real Schmidt semi-normalised harmonics, lm = l(l+1)+m, without trigonometry:
+// sin^m(theta) cos(m phi) = Re (mu + i eta)^m, sin^m(theta) sin(m phi) = Im (mu + i eta)^m, and
+// P_l^m(xi) = sin^m(theta) T_l^m(xi) with T_m^m = (2m-1)!!, T_{m+1}^m = (2m+1) xi T_m^m,
+// (l-m) T_l^m = (2l-1) xi T_{l-1}^m - (l+m-1) T_{l-2}^m  (no Condon-Shortley phase; R10).
+static void host_ylm(double mu, double eta, double xi, int L, double *y)
+{
+    double re = 1.0, im = 0.0, dfact = 1.0;
+    for (int m = 0; m <= L; ++m) {
+        if (m > 0) {
+            double nre = re * mu - im * eta, nim = re * eta + im * mu;
+            re = nre; im = nim;
+            dfact *= (2.0 * m - 1.0);
+        }
+        double t2 = 0.0, t1 = 0.0;
+        for (int l = m; l <= L; ++l) {
+            double t;
+            if (l == m) t = dfact;
+            else if (l == m + 1) t = (2.0 * m + 1.0) * xi * t1;
+            else t = ((2.0 * l - 1.0) * xi * t1 - (l + m - 1.0) * t2) / (double)(l - m);
+            t2 = t1; t1 = t;
+            if (m == 0) { y[l * (l + 1)] = t; continue; }
+            double f = 2.0;                       // 2 (l-m)!/(l+m)!
+            for (int s = l - m + 1; s <= l + m; ++s) f /= (double)s;
+            double nrm = std::sqrt(f);
+            y[l * (l + 1) + m] = nrm * t * re;
+            y[l * (l + 1) - m] = nrm * t * im;
+        }
+    }
+}
+
+static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L, int n_ang)
+{
+    Layout l;
+    const size_t nv = (size_t)m->nx * m->ny * m->nz;
+    const int MP = dos_mpad(L), per = n_ang / 8;
+    const int ntj = (m->ny + DOS_TJ - 1) / DOS_TJ, ntk = (m->nz + DOS_TK - 1) / DOS_TK;
+    const int ag = dos_sweep_angles_per_warp(per, L);
+    const int n_grp = ag ? per / ag : 1;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    l.phi_u = take(sizeof(float) * G * nv);
+    l.phi_all = take(sizeof(float) * G * nv * MP);
+    l.qfix = take(sizeof(float) * nv * MP);
+    l.q = take(sizeof(float) * nv * MP);
+    l.fy = take(sizeof(float) * (size_t)n_ang * ntj * m->nz * m->nx);
+    l.fz = take(sizeof(float) * (size_t)n_ang * ntk * m->ny * m->nx);
+    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * n_grp);
+    l.queue = take(sizeof(int) * 4);
+    l.items = take(sizeof(int) * (size_t)8 * ntj * ntk);
+    l.mat = take(nv);
+    l.dose_acc = take(sizeof(float) * nv);
+    l.sig_t = take(sizeof(float) * G * n_mat);          // stored [G][n_mat]
+    l.sig_s = take(sizeof(float) * (size_t)n_mat * (n_leg + 1) * G * G);
+    l.kerma = take(sizeof(float) * n_mat * G);
+    l.m2d = take(sizeof(float) * (size_t)n_ang * MP);
+    l.d2m = take(sizeof(float) * (size_t)n_ang * MP);
+    l.cdd = take(sizeof(float) * per * 4);
+    l.spectrum = take(sizeof(double) * G);
+    l.errflag = take(sizeof(int) * 4);
+    l.total = off;
+    return l;
+}
+
+static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos_quadrature *q, int P_L)
+{
+    if (!mesh || !xs || !q) return fail(nullptr, DOS_ERR_INVALID_ARG, "null argument");
+    if (mesh->nx < 1 || mesh->ny < 1 || mesh->nz < 1 || !(mesh->dx > 0) || !(mesh->dy > 0) || !(mesh->dz > 0))
+        return fail(nullptr, DOS_ERR_INVALID_ARG, "mesh sizes and spacings must be positive");
+    if ((size_t)mesh->nx * mesh->ny * mesh->nz >= ((size_t)1 << 31))
+        return fail(nullptr, DOS_ERR_UNSUPPORTED, "more than 2^31 voxels");
+    if (xs->n_mat < 1 || xs->n_mat > DOS_MAX_MAT) return fail(nullptr, DOS_ERR_UNSUPPORTED, "n_mat must be 1..16");
+    if (xs->n_group < 1 || xs->n_leg < 0 || !xs->sigma_t || !xs->sigma_s || !xs->kerma)
+        return fail(nullptr, DOS_ERR_INVALID_ARG, "bad cross-section table");
+    if (P_L < 0 || P_L > xs->n_leg) return fail(nullptr, DOS_ERR_SHAPE, "P_L must be 0..n_leg");
+    if (P_L > DOS_MAX_L) return fail(nullptr, DOS_ERR_UNSUPPORTED, "P_L > 5");
+    if (q->n_ang < 8 || q->n_ang % 8 || !q->mu || !q->eta || !q->xi || !q->w)
+        return fail(nullptr, DOS_ERR_INVALID_ARG, "n_ang must be a positive multiple of 8");
+    if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L) == 0)
+        return fail(nullptr, DOS_ERR_UNSUPPORTED, "angles per octant cannot be split over <= 12 warps of <= 4 angles");
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs, const dos_quadrature *quad,
+                                          int32_t P_L, int32_t n_batch, size_t *bytes_out)
+{
+    if (!bytes_out) return fail(nullptr, DOS_ERR_INVALID_ARG, "bytes_out is null");
+    dos_status s = check_inputs(mesh, xs, quad, P_L);
+    if (s != DOS_OK) return s;
+    if (n_batch != 1) return fail(nullptr, DOS_ERR_UNSUPPORTED, "n_batch must be 1");
+    *bytes_out = make_layout(mesh, xs->n_mat, xs->n_group, xs->n_leg, P_L, quad->n_ang).total;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint8_t *d_material_ids,
+                                 const dos_xs *xs, const dos_quadrature *quad, int32_t P_L, void *d_workspace,
+                                 size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return fail(nullptr, DOS_ERR_INVALID_ARG, "out is null");
+    *out = nullptr;
+    dos_status s = check_inputs(mesh, xs, quad, P_L);
+    if (s != DOS_OK) return s;
+    if (!d_material_ids || !d_workspace) return fail(nullptr, DOS_ERR_INVALID_ARG, "null device pointer");
+    if (((uintptr_t)d_workspace) & 255) return fail(nullptr, DOS_ERR_INVALID_ARG, "workspace not 256-byte aligned");
+    const int G = xs->n_group, n_mat = xs->n_mat, n_leg = xs->n_leg, L = P_L, n_ang = quad->n_ang, per = n_ang / 8;
+    const int M = (L + 1) * (L + 1), MP = dos_mpad(L);
+    // ---- table checks ----
+    for (int i = 0; i < n_mat * G; ++i)
+        if (!(xs->sigma_t[i] > 0.f)) return fail(nullptr, DOS_ERR_INVALID_ARG, "sigma_t must be > 0");
+    for (int m = 0; m < n_mat; ++m)
+        for (int l = 0; l <= n_leg; ++l)
+            for (int gf = 0; gf < G; ++gf)
+                for (int gt = 0; gt < gf; ++gt)
+                    if (xs->sigma_s[(((size_t)m * (n_leg + 1) + l) * G + gf) * G + gt] != 0.f)
+                        return fail(nullptr, DOS_ERR_INVALID_ARG, "sigma_s has upscatter (to < from) entries");
+    double wsum = 0.0;
+    for (int n = 0; n < n_ang; ++n) wsum += quad->w[n];
+    if (std::fabs(wsum - 1.0) > 1e-5) return fail(nullptr, DOS_ERR_INVALID_ARG, "quadrature weights must sum to 1");
+    for (int o = 0; o < 8; ++o)
+        for (int t = 0; t < per; ++t) {
+            const int n = o * per + t;
+            const float ex = (o & 1) ? -quad->mu[t] : quad->mu[t], ey = (o & 2) ? -quad->eta[t] : quad->eta[t],
+                        ez = (o & 4) ? -quad->xi[t] : quad->xi[t];
+            if (!(quad->mu[t] > 0.f && quad->eta[t] > 0.f && quad->xi[t] > 0.f) || quad->mu[n] != ex ||
+                quad->eta[n] != ey || quad->xi[n] != ez || quad->w[n] != quad->w[t])
+                return fail(nullptr, DOS_ERR_INVALID_ARG, "quadrature is not octant-major / octant-symmetric");
+        }
+    Layout lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang);
+    if (workspace_bytes < lay.total) return fail(nullptr, DOS_ERR_SHAPE, "workspace too small");
+
+    dos_ctx *c = new (std::nothrow) dos_ctx();
+    if (!c) return fail(nullptr, DOS_ERR_NOMEM, "out of host memory");
+    c->mesh = *mesh;
+    c->n_mat = n_mat; c->G = G; c->n_leg = n_leg; c->L = L; c->M = M; c->MP = MP; c->n_ang = n_ang; c->per_oct = per;
+    c->ntj = (mesh->ny + DOS_TJ - 1) / DOS_TJ;
+    c->ntk = (mesh->nz + DOS_TK - 1) / DOS_TK;
+    c->n_items = 8 * c->ntj * c->ntk;
+    c->ag = dos_sweep_angles_per_warp(per, L);
+    c->n_grp = per / c->ag;
+    c->chunk = mesh->nx <= 64 ? 8 : 16;
+    c->nv = (size_t)mesh->nx * mesh->ny * mesh->nz;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->d_mat = d_material_ids;
+    c->ws = (char *)d_workspace;
+    c->lay = lay;
+    c->state = 0;
+    c->have_dose_acc = false;
+    c->profile = false;
+    c->acc_ms[0] = c->acc_ms[1] = 0.0;
+    c->acc_n[0] = c->acc_n[1] = 0;
+    c->launches = 0;
+
+    // ---- host tables ----
+    std::vector<float> sig_t_gm((size_t)G * n_mat);
+    for (int m = 0; m < n_mat; ++m)
+        for (int g = 0; g < G; ++g) sig_t_gm[(size_t)g * n_mat + m] = xs->sigma_t[(size_t)m * G + g];
+    c->band_lo.assign(G, 0);
+    for (int g = 0; g < G; ++g) {
+        int lo = g;
+        for (int gp = g - 1; gp >= 0; --gp)
+            for (int m = 0; m < n_mat; ++m)
+                for (int l = 0; l <= L; ++l)
+                    if (xs->sigma_s[(((size_t)m * (n_leg + 1) + l) * G + gp) * G + g] != 0.f) lo = gp;
+        c->band_lo[g] = lo;
+    }
+    std::vector<float> m2d((size_t)n_ang * MP, 0.f), d2m((size_t)n_ang * MP, 0.f), cdd((size_t)per * 4);
+    double y[64];
+    for (int n = 0; n < n_ang; ++n) {
+        host_ylm((double)quad->mu[n], (double)quad->eta[n], (double)quad->xi[n], L, y);
+        for (int l = 0; l <= L; ++l)
+            for (int mm = -l; mm <= l; ++mm) {
+                const int lm = l * (l + 1) + mm;
+                m2d[(size_t)n * MP + lm] = (float)((2.0 * l + 1.0) * y[lm]);
+                d2m[(size_t)n * MP + lm] = (float)((double)quad->w[n] * y[lm]);
+            }
+    }
+    for (int t = 0; t < per; ++t) {
+        const double cx = 2.0 * std::fabs((double)quad->mu[t]) / mesh->dx, cy = 2.0 * std::fabs((double)quad->eta[t]) / mesh->dy,
+                     cz = 2.0 * std::fabs((double)quad->xi[t]) / mesh->dz;
+        cdd[t * 4 + 0] = (float)cx; cdd[t * 4 + 1] = (float)cy; cdd[t * 4 + 2] = (float)cz;
+        cdd[t * 4 + 3] = (float)(cx + cy + cz);
+    }
+    // work items, tile-diagonal major: every item's upwind tiles (tj-1,tk), (tj,tk-1) come earlier
+    std::vector<int> items;
+    items.reserve(c->n_items);
+    for (int d = 0; d <= c->ntj + c->ntk - 2; ++d)
+        for (int tj = 0; tj < c->ntj; ++tj) {
+            const int tk = d - tj;
+            if (tk < 0 || tk >= c->ntk) continue;
+            for (int o = 0; o < 8; ++o) items.push_back(o | (tj << 3) | (tk << 17));
+        }
+
+    auto up = [&](size_t off, const void *src, size_t bytes) {
+        return cudaMemcpyAsync(c->ws + off, src, bytes, cudaMemcpyHostToDevice, c->stream);
+    };
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = up(lay.sig_t, sig_t_gm.data(), sizeof(float) * sig_t_gm.size());
+    if (e == cudaSuccess) e = up(lay.sig_s, xs->sigma_s, sizeof(float) * (size_t)n_mat * (n_leg + 1) * G * G);
+    if (e == cudaSuccess) e = up(lay.kerma, xs->kerma, sizeof(float) * n_mat * G);
+    if (e == cudaSuccess) e = up(lay.m2d, m2d.data(), sizeof(float) * m2d.size());
+    if (e == cudaSuccess) e = up(lay.d2m, d2m.data(), sizeof(float) * d2m.size());
+    if (e == cudaSuccess) e = up(lay.cdd, cdd.data(), sizeof(float) * cdd.size());
+    if (e == cudaSuccess) e = up(lay.items, items.data(), sizeof(int) * items.size());
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.errflag, 0, sizeof(int) * 4, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // host vectors go out of scope
+    if (e == cudaSuccess) e = dos_sweep_grid(L, c->ag, per, n_mat, c->n_items, &c->grid);
+    if (e != cudaSuccess) {
+        std::string msg = std::string("dos_create: ") + cudaGetErrorString(e);
+        delete c;
+        return fail(nullptr, DOS_ERR_CUDA, msg);
+    }
+    *out = c;
+    return DOS_OK;
+}
+
+static MeshDev mesh_dev(const dos_mesh &m)
+{
+    MeshDev d;
+    d.nx = m.nx; d.ny = m.ny; d.nz = m.nz;
+    d.dx = m.dx; d.dy = m.dy; d.dz = m.dz;
+    d.x0 = m.x0; d.y0 = m.y0; d.z0 = m.z0;
+    return d;
+}
+
+static SourceDev source_dev(const dos_source &s)
+{
+    SourceDev d;
+    for (int i = 0; i < 3; ++i) { d.pos[i] = s.pos[i]; d.axis[i] = s.axis[i]; d.up[i] = s.up[i]; }
+    d.side[0] = s.axis[1] * s.up[2] - s.axis[2] * s.up[1];
+    d.side[1] = s.axis[2] * s.up[0] - s.axis[0] * s.up[2];
+    d.side[2] = s.axis[0] * s.up[1] - s.axis[1] * s.up[0];
+    d.tan_fan = s.tan_half_fan; d.tan_cone = s.tan_half_cone; d.isotropic = s.isotropic;
+    return d;
+}
+
+// optional CUDA-event bracket around one launch (option "profile")
+static void prof_begin(dos_ctx *c, int kind)
+{
+    if (!c->profile) return;
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+    c->ev.push_back(a); c->ev.push_back(b); c->ev_kind.push_back(kind);
+    cudaEventRecord(a, c->stream);
+}
+static void prof_end(dos_ctx *c)
+{
+    if (!c->profile || c->ev.empty()) return;
+    cudaEventRecord(c->ev.back(), c->stream);
+}
+static void prof_collect(dos_ctx *c)
+{
+    for (size_t i = 0; i < c->ev_kind.size(); ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->ev[2 * i], c->ev[2 * i + 1]) == cudaSuccess) {
+            c->acc_ms[c->ev_kind[i]] += ms;
+            c->acc_n[c->ev_kind[i]] += 1;
+        }
+        cudaEventDestroy(c->ev[2 * i]);
+        cudaEventDestroy(c->ev[2 * i + 1]);
+    }
+    c->ev.clear();
+    c->ev_kind.clear();
+}
+
+extern "C" dos_status dos_set_material_host(dos_ctx *c, const uint8_t *h_material_ids)
+{
+    if (!c || !h_material_ids) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    CUDA_TRY(c, cudaMemcpyAsync(c->ws + c->lay.mat, h_material_ids, c->nv, cudaMemcpyHostToDevice, c->stream));
+    c->d_mat = (const uint8_t *)(c->ws + c->lay.mat);
+    c->state = 0;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_uncollided(dos_ctx *c, const dos_source *source, const float *spectrum, float *d_phi_u_out)
+{
+    if (!c || !source || !spectrum) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    auto dot = [](const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; };
+    if (!source->isotropic) {
+        if (std::fabs(dot(source->axis, source->axis) - 1.0) > 1e-9 || std::fabs(dot(source->up, source->up) - 1.0) > 1e-9 ||
+            std::fabs(dot(source->axis, source->up)) > 1e-9)
+            return fail(c, DOS_ERR_INVALID_ARG, "axis and up must be orthonormal");
+        if (!(source->tan_half_fan >= 0.0) || !(source->tan_half_cone >= 0.0))
+            return fail(c, DOS_ERR_INVALID_ARG, "collimation tangents must be >= 0");
+    }
+    // a source closer than 1e-9 cm to a voxel centre has no defined direction (1/r^2 singular)
+    {
+        const dos_mesh &m = c->mesh;
+        const double fx = (source->pos[0] - m.x0) / m.dx - 0.5, fy = (source->pos[1] - m.y0) / m.dy - 0.5,
+                     fz = (source->pos[2] - m.z0) / m.dz - 0.5;
+        const double rx = std::nearbyint(fx), ry = std::nearbyint(fy), rz = std::nearbyint(fz);
+        if (rx >= 0 && rx < m.nx && ry >= 0 && ry < m.ny && rz >= 0 && rz < m.nz) {
+            const double ex = (fx - rx) * m.dx, ey = (fy - ry) * m.dy, ez = (fz - rz) * m.dz;
+            if (std::sqrt(ex * ex + ey * ey + ez * ez) < 1e-9)
+                return fail(c, DOS_ERR_INVALID_ARG, "source coincides with a voxel centre");
+        }
+    }
+    std::vector<double> sp(c->G);
+    for (int g = 0; g < c->G; ++g) {
+        if (!(spectrum[g] >= 0.f)) return fail(c, DOS_ERR_INVALID_ARG, "spectrum must be >= 0");
+        sp[g] = (double)spectrum[g];
+    }
+    c->src = *source;
+    CUDA_TRY(c, cudaMemcpyAsync(c->ws + c->lay.spectrum, sp.data(), sizeof(double) * c->G, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));   // sp is a stack-lifetime buffer
+    float *phi_u = (float *)(c->ws + c->lay.phi_u);
+    prof_begin(c, 1);
+    CUDA_TRY(c, dos_launch_raytrace(mesh_dev(c->mesh), source_dev(*source), c->d_mat, c->n_mat, c->G,
+                                    (const float *)(c->ws + c->lay.sig_t), (const double *)(c->ws + c->lay.spectrum),
+                                    phi_u, (int *)(c->ws + c->lay.errflag), c->stream));
+    prof_end(c);
+    c->launches += 1;
+    if (d_phi_u_out)
+        CUDA_TRY(c, cudaMemcpyAsync(d_phi_u_out, phi_u, sizeof(float) * c->G * c->nv, cudaMemcpyDeviceToDevice, c->stream));
+    c->state = 1;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
+{
+    if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
+    if (c->state < 1) return fail(c, DOS_ERR_STATE, "dos_solve before dos_uncollided");
+    if (n_iter < 1) return fail(c, DOS_ERR_INVALID_ARG, "n_iter must be >= 1");
+    const size_t nvm = c->nv * c->MP;
+    float *phi_u = (float *)(c->ws + c->lay.phi_u), *phi_all = (float *)(c->ws + c->lay.phi_all);
+    float *qfix = (float *)(c->ws + c->lay.qfix), *q = (float *)(c->ws + c->lay.q);
+    const float *sig_s = (const float *)(c->ws + c->lay.sig_s);
+    int *done = (int *)(c->ws + c->lay.done), *queue = (int *)(c->ws + c->lay.queue);
+    const MeshDev md = mesh_dev(c->mesh);
+    const SourceDev sd = source_dev(c->src);
+    SweepArgs a;
+    a.nx = c->mesh.nx; a.ny = c->mesh.ny; a.nz = c->mesh.nz;
+    a.ntj = c->ntj; a.ntk = c->ntk; a.n_items = c->n_items; a.per_oct = c->per_oct; a.n_grp = c->n_grp;
+    a.chunk = c->chunk; a.n_mat = c->n_mat;
+    a.items = (const int *)(c->ws + c->lay.items);
+    a.Q = q; a.mat = c->d_mat;
+    a.m2d = (const float *)(c->ws + c->lay.m2d); a.d2m = (const float *)(c->ws + c->lay.d2m);
+    a.cdd = (const float *)(c->ws + c->lay.cdd);
+    a.fy = (float *)(c->ws + c->lay.fy); a.fz = (float *)(c->ws + c->lay.fz);
+    a.done = done; a.queue = queue;
+    for (int g = 0; g < c->G; ++g) {
+        float *phi = phi_all + (size_t)g * nvm;
+        CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
+                                            phi_all, qfix, c->stream));
+        c->launches += 1;
+        a.phi = phi;
+        a.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
+        for (int it = 0; it < n_iter; ++it) {
+            CUDA_TRY(c, dos_launch_source_update(c->nv, c->d_mat, c->G, c->n_leg, c->L, g, sig_s, qfix, phi, q, it == 0,
+                                                 done, c->n_items * c->n_grp, queue, c->stream));
+            prof_begin(c, 0);
+            CUDA_TRY(c, dos_launch_sweep(a, c->L, c->ag, c->grid, c->stream));
+            prof_end(c);
+            c->launches += 2;
+        }
+    }
+    c->state = 2;
+    return DOS_OK;
+}
+
+static dos_status check_device_flags(dos_ctx *c)
+{
+    int h[4] = {0, 0, 0, 0};
+    CUDA_TRY(c, cudaMemcpyAsync(h, c->ws + c->lay.errflag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (h[0]) return fail(c, DOS_ERR_INVALID_ARG, "material id >= n_mat met on the device");
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_fluence(dos_ctx *c, float *d_phi_collided, float *d_phi_total)
+{
+    if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
+    if (c->state < 2) return fail(c, DOS_ERR_STATE, "dos_fluence before dos_solve");
+    CUDA_TRY(c, dos_launch_fluence(c->nv, c->G, c->MP, (const float *)(c->ws + c->lay.phi_u),
+                                   (const float *)(c->ws + c->lay.phi_all), d_phi_collided, d_phi_total, c->stream));
+    c->launches += 1;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_dose(dos_ctx *c, float *d_dose, int32_t accumulate)
+{
+    if (!c || !d_dose) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    if (c->state < 2) return fail(c, DOS_ERR_STATE, "dos_dose before dos_solve");
+    CUDA_TRY(c, dos_launch_dose(c->nv, c->d_mat, c->n_mat, c->G, c->MP, (const float *)(c->ws + c->lay.kerma),
+                                (const float *)(c->ws + c->lay.phi_u), (const float *)(c->ws + c->lay.phi_all), d_dose,
+                                accumulate, c->stream));
+    c->launches += 1;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_dose_host(dos_ctx *c, float *h_dose, int32_t accumulate)
+{
+    if (!c || !h_dose) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    float *acc = (float *)(c->ws + c->lay.dose_acc);
+    dos_status s = dos_dose(c, acc, accumulate && c->have_dose_acc);
+    if (s != DOS_OK) return s;
+    c->have_dose_acc = true;
+    CUDA_TRY(c, cudaMemcpyAsync(h_dose, acc, sizeof(float) * c->nv, cudaMemcpyDeviceToHost, c->stream));
+    return check_device_flags(c);
+}
+
+extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value)
+{
+    if (!c || !name) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    if (!strcmp(name, "sweep_chunk")) {
+        if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_chunk must be >= 1");
+        c->chunk = (int)value;
+    } else if (!strcmp(name, "profile")) {
+        c->profile = value != 0;
+    } else if (!strcmp(name, "sweep_grid")) {
+        if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_grid must be >= 1");
+        c->grid = (int)(value < c->n_items ? value : c->n_items);
+    } else {
+        return fail(c, DOS_ERR_INVALID_ARG, std::string("unknown option ") + name);
+    }
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_profile(dos_ctx *c, dos_profile_t *out)
+{
+    if (!c || !out) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    prof_collect(c);
+    out->sweep_ms = c->acc_ms[0]; out->sweep_launches = c->acc_n[0];
+    out->raytrace_ms = c->acc_ms[1]; out->raytrace_launches = c->acc_n[1];
+    out->kernel_launches = c->launches;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_profile_reset(dos_ctx *c)
+{
+    if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    prof_collect(c);
+    c->acc_ms[0] = c->acc_ms[1] = 0.0;
+    c->acc_n[0] = c->acc_n[1] = 0;
+    c->launches = 0;
+    return DOS_OK;
+}
+
+extern "C" void dos_destroy(dos_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    prof_collect(c);
+    delete c;
+}
+
+extern "C" const char *dos_last_error(const dos_ctx *c) { return c ? c->err.c_str() : g_err.c_str(); }

@@ -1,0 +1,42 @@
+// dos_internal.h -- shared between the translation units of libdos (CUDA path only).
+// Nothing here is used by, or taken from, oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define DOS_MAX_MAT 16      // material ids (ray-trace per-material path-length slots in shared memory)
+#define DOS_MAX_L 5         // highest P_L
+#define DOS_TJ 8            // sweep tile: lanes of a warp cover TJ x TK (j,k) columns and march along x
+#define DOS_TK 4
+#define DOS_SKEW (DOS_TJ + DOS_TK - 2)
+
+// number of moments (L+1)^2 padded to a multiple of 4 so that a cell's moments are whole float4s
+static inline __host__ __device__ int dos_mpad(int L) { return (((L + 1) * (L + 1)) + 3) & ~3; }
+
+// Arguments of one sweep launch (all 8 octants, one energy group, one source iteration).
+struct SweepArgs {
+    int nx, ny, nz;
+    int ntj, ntk;            // tiles along j and k
+    int n_items;             // 8 * ntj * ntk work items (octant, tile)
+    int per_oct;             // angles per octant (A)
+    int n_grp;               // angle groups = warps per CTA (A / AG)
+    int chunk;               // cells along x between flag publications
+    int n_mat;
+    const int *items;        // [n_items] packed (octant | tj << 3 | tk << 17), dependency-safe order
+    const float *Q;          // [Nv][MP] frozen source moments
+    float *phi;              // [Nv][MP] accumulates w Y psi (zeroed before the launch)
+    const uint8_t *mat;      // [Nv]
+    const float *sig_t;      // [n_mat] total cross section of this group
+    const float *m2d;        // [8][A][MP] (2l+1) Y_lm(Omega_n)
+    const float *d2m;        // [8][A][MP] w_n Y_lm(Omega_n)
+    const float *cdd;        // [A][4] cx, cy, cz, cx+cy+cz  (2|Omega_d|/Delta_d; same for all octants)
+    float *fy;               // [8][A][ntj][nz'][nx'] y-face fluxes leaving tile row tj (oriented indices)
+    float *fz;               // [8][A][ntk][ny'][nx'] z-face fluxes leaving tile row tk
+    int *done;               // [n_items (by id)][n_grp] cells along x finished and published
+    int *queue;              // work-queue head
+};
+
+// dos_sweep.cu
+cudaError_t dos_launch_sweep(const SweepArgs &a, int L, int ang_per_warp, int grid, cudaStream_t s);
+int dos_sweep_angles_per_warp(int per_oct, int L);
+cudaError_t dos_sweep_grid(int L, int ang_per_warp, int per_oct, int n_mat, int n_items, int *grid_out);
