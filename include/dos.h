@@ -132,6 +132,10 @@ dos_status dos_dose(dos_ctx *ctx, float *d_dose, int32_t accumulate);
  * accumulate != 0 the device-side running sum kept in the workspace is extended and returned. */
 dos_status dos_dose_host(dos_ctx *ctx, float *h_dose, int32_t accumulate);
 
+/* Synchronises the stream and reports what the kernels flagged on the device since dos_create:
+ * a material id >= n_mat (DOS_ERR_INVALID_ARG), a stuck sweep hand-off or a CUDA fault (DOS_ERR_CUDA). */
+dos_status dos_check(dos_ctx *ctx);
+
 /* Tuning / measurement knobs (all optional).
  *   "sweep_chunk"   cells along x between face-flux hand-offs of neighbouring tiles (>= 1)
  *   "profile"       1: bracket every sweep and ray-trace launch with CUDA events (see dos_profile)  */

@@ -40,6 +40,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_harmonics.restype = None
         _lib.orc_uncollided.restype = C.c_int
+        _lib.orc_uncollided_cells.restype = C.c_int
         _lib.orc_first_collision.restype = None
         _lib.orc_sweep.restype = C.c_int
         _lib.orc_solve.restype = C.c_int
@@ -87,6 +88,25 @@ def uncollided(mesh, material, sigma_t, source, spectrum, want_path=False):
         raise ValueError("source coincides with a voxel centre")
     phi = phi.reshape((G,) + mat.shape)
     return (phi, path.reshape(mat.shape)) if want_path else phi
+
+
+def uncollided_at(mesh, material, sigma_t, source, spectrum, cells):
+    """phi_u [G][len(cells)] for the listed flat voxel indices (k*ny*nx + j*nx + i) only."""
+    sig = _d(sigma_t)
+    n_mat, G = sig.shape
+    mat = np.ascontiguousarray(material, dtype=np.uint8)
+    idx = np.ascontiguousarray(cells, dtype=np.int64)
+    assert idx.min() >= 0 and idx.max() < mat.size
+    phi = np.zeros((G, idx.size))
+    pos, axis, up = _d(source["pos"]), _d(source["axis"]), _d(source["up"])
+    ms = _mesh(mesh)
+    err = lib().orc_uncollided_cells(C.byref(ms), _p(mat), C.c_int(n_mat), C.c_int(G), _p(sig), _p(pos), _p(axis),
+                                     _p(up), C.c_double(source["tan_half_fan"]), C.c_double(source["tan_half_cone"]),
+                                     C.c_int(source["isotropic"]), _p(_d(spectrum)), _p(idx), C.c_longlong(idx.size),
+                                     _p(phi))
+    if err:
+        raise ValueError("source coincides with a voxel centre")
+    return phi
 
 
 def sweep(mesh, material, sig_t_g, quad, L, Q, reflective=False, bnd_state=None, want_leakage=False,

@@ -157,8 +157,35 @@ static int inside_beam(const double d[3], const double axis[3], const double up[
     return fabs(u) <= a * tan_cone && fabs(v) <= a * tan_fan;
 }
 
-/* phi_u^g(c) = S_g exp(-tau_g) / (4 pi r^2) inside the beam, 0 outside (R7).
- * sigma_t [n_mat][G]; phi_u out [G][Nv]; optional path_total out [Nv] (in-mesh geometric length). */
+/* phi_u^g(c) = S_g exp(-tau_g) / (4 pi r^2) inside the beam, 0 outside (R7), for ONE voxel.
+ * out[g] (stride `stride` doubles between groups). Returns 1 if the source sits on the voxel centre. */
+static int uncollided_cell(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, const double *sigma_t,
+                           const double *pos, const double *axis, const double *up, double tan_fan,
+                           double tan_cone, int isotropic, const double *spectrum, long long cell,
+                           double *out, size_t stride, double *path_total, double *len_mat, double *abuf)
+{
+    int i = (int)(cell % ms->nx), j = (int)((cell / ms->nx) % ms->ny),
+        k = (int)(cell / ((long long)ms->nx * ms->ny));
+    double c[3] = {ms->x0 + (i + 0.5) * ms->dx, ms->y0 + (j + 0.5) * ms->dy, ms->z0 + (k + 0.5) * ms->dz};
+    double d[3] = {c[0] - pos[0], c[1] - pos[1], c[2] - pos[2]};
+    double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    if (r2 < 1e-18) return 1;
+    if (!inside_beam(d, axis, up, tan_fan, tan_cone, isotropic)) {
+        for (int g = 0; g < G; ++g) out[(size_t)g * stride] = 0.0;
+        if (path_total) *path_total = 0.0;
+        return 0;
+    }
+    double tot = path_lengths(ms, mat, n_mat, pos, c, len_mat, abuf);
+    if (path_total) *path_total = tot;
+    for (int g = 0; g < G; ++g) {
+        double tau = 0.0;
+        for (int m = 0; m < n_mat; ++m) tau += sigma_t[(size_t)m * G + g] * len_mat[m];
+        out[(size_t)g * stride] = spectrum[g] * exp(-tau) / (4.0 * ORC_PI * r2);
+    }
+    return 0;
+}
+
+/* All voxels. sigma_t [n_mat][G]; phi_u out [G][Nv]; optional path_total out [Nv] (in-mesh length). */
 int orc_uncollided(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, const double *sigma_t,
                    const double *pos, const double *axis, const double *up, double tan_fan,
                    double tan_cone, int isotropic, const double *spectrum, double *phi_u,
@@ -171,27 +198,34 @@ int orc_uncollided(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, con
         double *len_mat = (double *)malloc(sizeof(double) * (size_t)n_mat);
         double *abuf = (double *)malloc(sizeof(double) * (size_t)(ms->nx + ms->ny + ms->nz + 8));
 #pragma omp for schedule(dynamic, 64)
-        for (long long cell = 0; cell < (long long)nv; ++cell) {
-            int i = (int)(cell % ms->nx), j = (int)((cell / ms->nx) % ms->ny),
-                k = (int)(cell / ((long long)ms->nx * ms->ny));
-            double c[3] = {ms->x0 + (i + 0.5) * ms->dx, ms->y0 + (j + 0.5) * ms->dy,
-                           ms->z0 + (k + 0.5) * ms->dz};
-            double d[3] = {c[0] - pos[0], c[1] - pos[1], c[2] - pos[2]};
-            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-            if (r2 < 1e-18) { err = 1; continue; }
-            if (!inside_beam(d, axis, up, tan_fan, tan_cone, isotropic)) {
-                for (int g = 0; g < G; ++g) phi_u[(size_t)g * nv + cell] = 0.0;
-                if (path_total) path_total[cell] = 0.0;
-                continue;
-            }
-            double tot = path_lengths(ms, mat, n_mat, pos, c, len_mat, abuf);
-            if (path_total) path_total[cell] = tot;
-            for (int g = 0; g < G; ++g) {
-                double tau = 0.0;
-                for (int m = 0; m < n_mat; ++m) tau += sigma_t[(size_t)m * G + g] * len_mat[m];
-                phi_u[(size_t)g * nv + cell] = spectrum[g] * exp(-tau) / (4.0 * ORC_PI * r2);
-            }
-        }
+        for (long long cell = 0; cell < (long long)nv; ++cell)
+            if (uncollided_cell(ms, mat, n_mat, G, sigma_t, pos, axis, up, tan_fan, tan_cone, isotropic,
+                                spectrum, cell, phi_u + cell, nv, path_total ? path_total + cell : NULL,
+                                len_mat, abuf))
+                err = 1;
+        free(len_mat);
+        free(abuf);
+    }
+    return err;
+}
+
+/* The same for a list of voxels (flat indices cells[n_cells]); phi_u out [G][n_cells]. Used to check
+ * sampled voxels of meshes too large to trace in full. */
+int orc_uncollided_cells(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, const double *sigma_t,
+                         const double *pos, const double *axis, const double *up, double tan_fan,
+                         double tan_cone, int isotropic, const double *spectrum, const long long *cells,
+                         long long n_cells, double *phi_u)
+{
+    int err = 0;
+#pragma omp parallel
+    {
+        double *len_mat = (double *)malloc(sizeof(double) * (size_t)n_mat);
+        double *abuf = (double *)malloc(sizeof(double) * (size_t)(ms->nx + ms->ny + ms->nz + 8));
+#pragma omp for schedule(dynamic, 16)
+        for (long long t = 0; t < n_cells; ++t)
+            if (uncollided_cell(ms, mat, n_mat, G, sigma_t, pos, axis, up, tan_fan, tan_cone, isotropic,
+                                spectrum, cells[t], phi_u + t, (size_t)n_cells, NULL, len_mat, abuf))
+                err = 1;
         free(len_mat);
         free(abuf);
     }

@@ -5,3 +5,4 @@ binding of csrc/libdos.so (built in-tree with nvcc for sm_100a). There is no CPU
 """
 from . import inputs  # noqa: F401
 from . import dos  # noqa: F401
+from . import scan  # noqa: F401

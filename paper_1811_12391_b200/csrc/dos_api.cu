@@ -31,9 +31,10 @@ struct dos_ctx {
     int state;                   // 0 created, 1 uncollided done, 2 solved
     dos_source src;
     bool have_dose_acc;
-    bool profile;
+    bool profile, prof_open;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop); kind in ev_kind
     std::vector<int> ev_kind;     // 0 sweep, 1 ray trace
+    std::vector<cudaEvent_t> ev_pool;   // recycled events (creating one per launch would cost host time)
     double acc_ms[2];
     int64_t acc_n[2];
     int64_t launches;
@@ -203,7 +204,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->lay = lay;
     c->state = 0;
     c->have_dose_acc = false;
-    c->profile = false;
+    c->profile = false; c->prof_open = false;
     c->acc_ms[0] = c->acc_ms[1] = 0.0;
     c->acc_n[0] = c->acc_n[1] = 0;
     c->launches = 0;
@@ -295,15 +296,20 @@ static SourceDev source_dev(const dos_source &s)
 static void prof_begin(dos_ctx *c, int kind)
 {
     if (!c->profile) return;
-    cudaEvent_t a, b;
-    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
-    c->ev.push_back(a); c->ev.push_back(b); c->ev_kind.push_back(kind);
-    cudaEventRecord(a, c->stream);
+    cudaEvent_t e[2];
+    for (int i = 0; i < 2; ++i) {
+        if (!c->ev_pool.empty()) { e[i] = c->ev_pool.back(); c->ev_pool.pop_back(); }
+        else if (cudaEventCreate(&e[i]) != cudaSuccess) { c->prof_open = false; return; }
+    }
+    c->ev.push_back(e[0]); c->ev.push_back(e[1]); c->ev_kind.push_back(kind);
+    c->prof_open = true;
+    cudaEventRecord(e[0], c->stream);
 }
 static void prof_end(dos_ctx *c)
 {
-    if (!c->profile || c->ev.empty()) return;
+    if (!c->profile || !c->prof_open) return;
     cudaEventRecord(c->ev.back(), c->stream);
+    c->prof_open = false;
 }
 static void prof_collect(dos_ctx *c)
 {
@@ -313,8 +319,8 @@ static void prof_collect(dos_ctx *c)
             c->acc_ms[c->ev_kind[i]] += ms;
             c->acc_n[c->ev_kind[i]] += 1;
         }
-        cudaEventDestroy(c->ev[2 * i]);
-        cudaEventDestroy(c->ev[2 * i + 1]);
+        c->ev_pool.push_back(c->ev[2 * i]);
+        c->ev_pool.push_back(c->ev[2 * i + 1]);
     }
     c->ev.clear();
     c->ev_kind.clear();
@@ -395,6 +401,7 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
     a.cdd = (const float *)(c->ws + c->lay.cdd);
     a.fy = (float *)(c->ws + c->lay.fy); a.fz = (float *)(c->ws + c->lay.fz);
     a.done = done; a.queue = queue;
+    a.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
         CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
@@ -421,7 +428,14 @@ static dos_status check_device_flags(dos_ctx *c)
     CUDA_TRY(c, cudaMemcpyAsync(h, c->ws + c->lay.errflag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     if (h[0]) return fail(c, DOS_ERR_INVALID_ARG, "material id >= n_mat met on the device");
+    if (h[1]) return fail(c, DOS_ERR_CUDA, "sweep watchdog fired: a face-flux hand-off never arrived; results are invalid");
     return DOS_OK;
+}
+
+extern "C" dos_status dos_check(dos_ctx *c)
+{
+    if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
+    return check_device_flags(c);
 }
 
 extern "C" dos_status dos_fluence(dos_ctx *c, float *d_phi_collided, float *d_phi_total)
@@ -500,6 +514,7 @@ extern "C" void dos_destroy(dos_ctx *c)
     if (!c) return;
     cudaStreamSynchronize(c->stream);
     prof_collect(c);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
 }
 

@@ -9,6 +9,7 @@
 #define DOS_TJ 8            // sweep tile: lanes of a warp cover TJ x TK (j,k) columns and march along x
 #define DOS_TK 4
 #define DOS_SKEW (DOS_TJ + DOS_TK - 2)
+#define DOS_SPIN_LIMIT (1 << 22)   // polls of an upwind flag before the sweep declares itself stuck
 
 // number of moments (L+1)^2 padded to a multiple of 4 so that a cell's moments are whole float4s
 static inline __host__ __device__ int dos_mpad(int L) { return (((L + 1) * (L + 1)) + 3) & ~3; }
@@ -34,6 +35,7 @@ struct SweepArgs {
     float *fz;               // [8][A][ntk][ny'][nx'] z-face fluxes leaving tile row tk
     int *done;               // [n_items (by id)][n_grp] cells along x finished and published
     int *queue;              // work-queue head
+    int *abort_flag;         // set by the watchdog; every waiting warp then stops waiting
 };
 
 // dos_sweep.cu

@@ -150,11 +150,18 @@ __global__ void __launch_bounds__(384) sweep_kernel(const SweepArgs p)
             // ---- prefetch step t+1 (needs the upwind faces of cell t+1 of the lead lane) ----
             if (t + 1 < T) {
                 const int need = min(t + 2, nx);
+                int spins = 0;
                 while (avail < need) {
                     int ya = dep_y ? ld_acquire(up_y) : nx;
                     int za = dep_z ? ld_acquire(up_z) : nx;
                     avail = min(ya, za);
-                    if (avail < need) __nanosleep(40);
+                    if (avail < need) {
+                        __nanosleep(40);
+                        // watchdog: a hand-off that never arrives must not hang the GPU; the result is
+                        // then invalid and dos_check / dos_dose_host report DOS_ERR_CUDA
+                        if (++spins > DOS_SPIN_LIMIT) atomicExch(p.abort_flag, 1);
+                        if ((spins & 255) == 0 && ld_acquire(p.abort_flag)) avail = nx;
+                    }
                 }
                 const int ipn = t + 1 - skew;
                 if (valid && ipn >= 0 && ipn < nx) {

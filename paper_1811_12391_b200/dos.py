@@ -21,7 +21,7 @@ STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_
           -5: "DOS_ERR_CUDA", -6: "DOS_ERR_UNSUPPORTED"}
 
 EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_solve",
-           "dos_fluence", "dos_dose", "dos_dose_host", "dos_set_option", "dos_profile", "dos_profile_reset",
+           "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option", "dos_profile", "dos_profile_reset",
            "dos_destroy", "dos_last_error"]
 
 
@@ -67,6 +67,8 @@ _lib.dos_dose.restype = C.c_int
 _lib.dos_dose.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
 _lib.dos_dose_host.restype = C.c_int
 _lib.dos_dose_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+_lib.dos_check.restype = C.c_int
+_lib.dos_check.argtypes = [C.c_void_p]
 _lib.dos_set_option.restype = C.c_int
 _lib.dos_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
 _lib.dos_profile.restype = C.c_int
@@ -195,6 +197,9 @@ class Context:
         assert dose_host.dtype == np.float32 and dose_host.flags["C_CONTIGUOUS"]
         self._check(_lib.dos_dose_host(self.handle, dose_host.ctypes.data, int(bool(accumulate))))
 
+    def dos_check(self):
+        self._check(_lib.dos_check(self.handle))
+
     def dos_set_option(self, name, value):
         self._check(_lib.dos_set_option(self.handle, name.encode(), int(value)))
 
@@ -235,7 +240,7 @@ def run_problem(p, source_index=0, n_iter=None, device="cuda:0", ctx=None):
     ctx.dos_solve(p["n_iter"] if n_iter is None else n_iter)
     ctx.dos_fluence(pc, pt)
     ctx.dos_dose(d, False)
-    ctx.torch.cuda.synchronize(ctx.device)
+    ctx.dos_check()
     out = {"phi_u": pu.cpu().numpy(), "phi_c": pc.cpu().numpy(), "phi_total": pt.cpu().numpy(), "dose": d.cpu().numpy()}
     if own:
         ctx.close()

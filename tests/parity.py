@@ -1,0 +1,68 @@
+"""Error measures and tolerances of the GPU-vs-oracle parity tests (BASELINE.json north_star).
+
+  scalar fluence (total and collided, per group) and dose:
+      relative L2 error over all voxels  <= 1e-5
+      max relative error over voxels above 1e-6 of the field's peak  <= 1e-4
+  uncollided fluence: max relative error over voxels above 1e-6 of the group's peak <= 1e-6, and the
+      zero pattern (beam membership) must match exactly. The GPU stores fp32, so an oracle value below
+      the smallest normal fp32 (1.18e-38) may legitimately read back as 0 or as a denormal.
+"""
+import numpy as np
+
+TOL_L2 = 1e-5
+TOL_MAX = 1e-4
+TOL_UNCOLLIDED = 1e-6
+FLT_MIN = 1.1754943508222875e-38
+
+
+def field_errors(gpu, ref):
+    """(relL2, max rel error above 1e-6 of peak) of one field (any shape)."""
+    g = np.asarray(gpu, dtype=np.float64).ravel()
+    r = np.asarray(ref, dtype=np.float64).ravel()
+    peak = np.abs(r).max()
+    if peak == 0.0:
+        return (0.0 if not g.any() else np.inf), (0.0 if not g.any() else np.inf)
+    l2 = np.linalg.norm(g - r) / np.linalg.norm(r)
+    m = np.abs(r) > 1e-6 * peak
+    return l2, (np.abs(g - r)[m] / np.abs(r)[m]).max()
+
+
+def per_group_errors(gpu, ref):
+    errs = np.array([field_errors(gpu[g], ref[g]) for g in range(ref.shape[0])])
+    return errs[:, 0].max(), errs[:, 1].max()
+
+
+def assert_fluence_parity(gpu, ref, what):
+    l2, mx = per_group_errors(gpu, ref)
+    assert l2 <= TOL_L2 and mx <= TOL_MAX, f"{what}: relL2 {l2:.3e} (<= {TOL_L2}), max rel {mx:.3e} (<= {TOL_MAX})"
+    return l2, mx
+
+
+def assert_dose_parity(gpu, ref, what="dose"):
+    l2, mx = field_errors(gpu, ref)
+    assert l2 <= TOL_L2 and mx <= TOL_MAX, f"{what}: relL2 {l2:.3e}, max rel {mx:.3e}"
+    return l2, mx
+
+
+def assert_uncollided_parity(gpu, ref):
+    gpu = np.asarray(gpu)
+    ref = np.asarray(ref, dtype=np.float64)
+    # beam membership: exact zeros of the oracle are exact zeros on the GPU, and nothing else is zero
+    # unless the oracle's value is below fp32 range
+    assert not gpu[ref == 0.0].any(), "GPU has fluence outside the oracle's beam"
+    lost = (gpu == 0.0) & (ref != 0.0)
+    assert (np.abs(ref[lost]) < FLT_MIN).all(), "GPU has zeros inside the oracle's beam"
+    worst = 0.0
+    for g in range(ref.shape[0]):
+        _, mx = field_errors(gpu[g], ref[g])
+        worst = max(worst, mx)
+    assert worst <= TOL_UNCOLLIDED, f"uncollided max rel error {worst:.3e} (<= {TOL_UNCOLLIDED})"
+    return worst
+
+
+def assert_problem_parity(out, ref, name=""):
+    res = {"phi_u": assert_uncollided_parity(out["phi_u"], ref["phi_u"]),
+           "phi_c": assert_fluence_parity(out["phi_c"], ref["phi_c"], name + " collided fluence"),
+           "phi_total": assert_fluence_parity(out["phi_total"], ref["phi_total"], name + " total fluence"),
+           "dose": assert_dose_parity(out["dose"], ref["dose"], name + " dose")}
+    return res

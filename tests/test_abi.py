@@ -1,0 +1,132 @@
+"""CPU-only checks of the C-ABI boundary (include/dos.h <-> csrc/libdos.so <-> the Python binding).
+
+No compute call is made here: only symbol presence, struct layout, and the argument validation that
+runs on the host before any CUDA call.
+"""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "dos.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dos_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_1811_12391_b200 import dos
+    lib = C.CDLL(dos.library_path())
+    names = _declared()
+    assert {"dos_create", "dos_uncollided", "dos_solve", "dos_dose", "dos_destroy"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/dos.h but not exported"
+    assert sorted(dos.EXPORTS) == names, "binding's EXPORTS list and include/dos.h disagree"
+
+
+def test_library_is_sm100a_and_not_linked_to_the_oracle():
+    from paper_1811_12391_b200 import dos
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-lelf", dos.library_path()], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    ldd = subprocess.run(["ldd", dos.library_path()], capture_output=True, text=True).stdout
+    assert "oracle" not in ldd
+
+
+def test_product_sources_do_not_reference_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1811_12391_b200")
+    for d, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cpp")):
+                src = open(os.path.join(d, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle", src, flags=re.M), f
+                assert "dos_oracle" not in src and "libdos_oracle" not in src, f
+
+
+def _problem():
+    from paper_1811_12391_b200.inputs import make_problem
+    return make_problem("config1")
+
+
+def test_struct_layouts_match_the_header():
+    from paper_1811_12391_b200 import dos
+    assert C.sizeof(dos.dos_mesh) == 3 * 4 + 4 + 6 * 8          # 3 int32, pad, 6 double
+    assert C.sizeof(dos.dos_source) == 9 * 8 + 2 * 8 + 8        # 3x3 double, 2 double, int32 + pad
+    assert C.sizeof(dos.dos_xs) == 16 + 3 * 8
+    assert C.sizeof(dos.dos_quadrature) == 8 + 4 * 8
+
+
+def test_workspace_bytes_and_host_side_validation():
+    from paper_1811_12391_b200 import dos
+    p = _problem()
+    n = dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    nv = 16 ** 3
+    assert n >= 4 * nv * 4 * (p["n_group"] + 2)                  # moments of all groups + Q_fix + Q
+    with pytest.raises(dos.DosError) as e:
+        dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 3)
+    assert e.value.status == -2                                  # P_L > n_leg -> DOS_ERR_SHAPE
+    bad = dict(p["mesh"], nx=0)
+    with pytest.raises(dos.DosError) as e:
+        dos.dos_workspace_bytes(bad, p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 1)
+    assert e.value.status == -1
+    with pytest.raises(dos.DosError) as e:
+        dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 1, n_batch=2)
+    assert e.value.status == -6
+    q = {k: (v[:20] if k in ("mu", "eta", "xi", "w") else v) for k, v in p["quadrature"].items()}
+    with pytest.raises(dos.DosError) as e:
+        dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], q, 1)
+    assert e.value.status == -1                                  # n_ang not a multiple of 8
+
+
+def test_create_rejects_bad_tables_before_touching_cuda():
+    """dos_create validates host tables first; with fake (never dereferenced) device pointers the
+    failures below must come back as statuses, not crashes, on a box without a GPU."""
+    from paper_1811_12391_b200 import dos
+    lib = dos.raw()
+    p = _problem()
+    ms = dos._mesh_struct(p["mesh"])
+    h = C.c_void_p(None)
+    fake_dev = C.c_void_p(0x10000)          # 256-aligned, never dereferenced on these paths
+
+    def create(sigma_t=None, sigma_s=None, quad=None, ws=fake_dev, mat=fake_dev, nbytes=1 << 40):
+        t = dos._Tables(p["sigma_t"] if sigma_t is None else sigma_t, p["sigma_s"] if sigma_s is None else sigma_s,
+                        p["kerma"], p["quadrature"] if quad is None else quad)
+        st = lib.dos_create(C.byref(h), C.byref(ms), mat, C.byref(t.xs), C.byref(t.quad), 1, ws, nbytes, None)
+        return st, lib.dos_last_error(None).decode()
+
+    st, msg = create(sigma_t=np.zeros_like(p["sigma_t"]))
+    assert st == -1 and "sigma_t" in msg
+    up = p["sigma_s"].copy()
+    up[0, 0, 2, 1] = 0.1                                         # upscatter entry
+    st, msg = create(sigma_s=up)
+    assert st == -1 and "upscatter" in msg
+    q = dict(p["quadrature"])
+    q["w"] = q["w"] * np.float32(1.01)
+    st, msg = create(quad=q)
+    assert st == -1 and "sum to 1" in msg
+    q = dict(p["quadrature"])
+    q["mu"] = q["mu"][::-1].copy()
+    st, msg = create(quad=q)
+    assert st == -1 and "octant" in msg
+    st, msg = create(ws=C.c_void_p(0x10010))
+    assert st == -1 and "aligned" in msg
+    st, msg = create(mat=None)
+    assert st == -1
+    st, msg = create(nbytes=1024)
+    assert st == -2 and "workspace" in msg
+    assert h.value is None
+
+
+def test_null_context_calls_return_status():
+    from paper_1811_12391_b200 import dos
+    lib = dos.raw()
+    assert lib.dos_solve(None, 3) == -1
+    assert lib.dos_dose(None, None, 0) == -1
+    assert lib.dos_uncollided(None, None, None, None) == -1
+    assert lib.dos_check(None) == -1
+    lib.dos_destroy(None)                                        # no-op

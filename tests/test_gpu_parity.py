@@ -1,0 +1,237 @@
+"""GPU-vs-oracle parity of the whole hot path, through the C ABI (run on the B200 box: -m gpu).
+
+Every case builds one seeded problem (paper_1811_12391_b200.inputs), runs the fp64 oracle and the CUDA
+library on the same fp32-rounded tables and compares element by element with the tolerances of
+tests/parity.py (BASELINE.json north_star).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from parity import (assert_dose_parity, assert_fluence_parity, assert_problem_parity, assert_uncollided_parity,
+                    field_errors, per_group_errors)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dos():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1811_12391_b200 import dos as d
+    return d
+
+
+def _make(name, **ov):
+    from paper_1811_12391_b200.inputs import make_problem
+    return make_problem(name, **ov)
+
+
+# ---------------------------------------------------------------- element-by-element, small sizes --
+# Reduced versions of each config: same materials / xs model / quadrature / P_L / source geometry, mesh
+# sizes that span several 8x4 sweep tiles with ragged tails in j and k and an x length that is not a
+# multiple of the hand-off chunk.
+SMALL = [
+    ("config1", {}),                                                                    # the full config 1
+    ("config2", dict(nx=37, ny=21, nz=10, voxel=1.0, n_group=5, n_iter=6)),
+    ("config3", dict(nx=26, ny=20, nz=9, voxel=1.5, n_group=4, n_iter=3)),
+    ("config4", dict(nx=30, ny=27, nz=7, voxel=1.3, n_group=6, n_iter=4, n_pos=1)),
+    ("config5", dict(nx=19, ny=17, nz=21, voxel=1.9, n_group=3, n_iter=3)),
+    ("config2", dict(nx=5, ny=3, nz=2, voxel=7.0, n_group=3, n_iter=2, sn=2, pl=0)),     # one partial tile, S2/P0
+    ("config2", dict(nx=1, ny=1, nz=1, voxel=30.0, n_group=2, n_iter=2, sn=4, pl=1)),    # single voxel
+    ("config2", dict(nx=33, ny=9, nz=5, voxel=1.1, n_group=3, n_iter=3, sn=6, pl=2)),    # S6/P2 (M padded 9->12)
+    ("config4", dict(nx=18, ny=16, nz=8, voxel=2.0, n_group=4, n_iter=3, n_pos=1, sn=12, pl=4)),  # S12/P4
+]
+
+
+@pytest.mark.parametrize("name,ov", SMALL, ids=[f"{n}-{i}" for i, (n, _) in enumerate(SMALL)])
+def test_small_problem_parity(dos, orc, name, ov):
+    p = _make(name, **ov)
+    ref = orc.run_problem(p)
+    out = dos.run_problem(p)
+    assert_problem_parity(out, ref, name)
+
+
+def test_config2_full_parity(dos, orc):
+    """BASELINE.json configs[1] at full size and full iteration count."""
+    p = _make("config2")
+    ref = orc.run_problem(p)
+    out = dos.run_problem(p)
+    res = assert_problem_parity(out, ref, "config2")
+    print("config2 parity", res)
+
+
+# -------------------------------------------------- full mesh sizes, bench launch configuration --
+# The oracle cannot finish the full group/iteration count of configs 3-5 in test time, so the mesh,
+# quadrature and P_L (which fix tiles, warps, chunk and grid of every launch) are the full ones and
+# the group and iteration counts are cut. Every group/iteration is the same launch sequence.
+def test_config3_full_mesh_parity(dos, orc):
+    p = _make("config3", n_group=2, n_iter=2)
+    ref = orc.run_problem(p)
+    out = dos.run_problem(p)
+    assert_problem_parity(out, ref, "config3 mesh")
+
+
+def test_config4_full_mesh_two_positions_accumulate(dos, orc):
+    """256x256x64 abdomen phantom, S8/P3; two of the 36 source positions, doses summed (a9)."""
+    p = _make("config4", n_group=2, n_iter=1)
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    d = ctx.new_field(groups=False)
+    ref_sum = None
+    for n, s in enumerate((0, 13)):
+        ctx.dos_uncollided(p["sources"][s], p["spectrum"])
+        ctx.dos_solve(p["n_iter"])
+        ctx.dos_dose(d, accumulate=(n > 0))
+        r = orc.run_problem(p, source_index=s)
+        ref_sum = r["dose"] if ref_sum is None else ref_sum + r["dose"]
+    ctx.dos_check()
+    assert_dose_parity(d.cpu().numpy(), ref_sum, "scan dose (2 positions)")
+    ctx.close()
+
+
+@pytest.mark.skipif(not os.environ.get("DOS_FULL_ORACLE"), reason="needs ~45 GB host RAM and minutes of oracle time; "
+                    "set DOS_FULL_ORACLE=1 (result recorded in DESIGN.md)")
+def test_config5_full_mesh_parity_opt_in(dos, orc):
+    p = _make("config5", n_group=1, n_iter=1)
+    ref = orc.run_problem(p)
+    out = dos.run_problem(p)
+    assert_problem_parity(out, ref, "config5 mesh")
+
+
+def test_config5_full_mesh_properties(dos, orc):
+    """256^3, S16/P5 in the bench launch configuration. Properties that hold at any size:
+    (i) uncollided fluence of sampled voxels equals the oracle's (the oracle traces just those voxels:
+        a sub-mesh cannot be used, the ray crosses the whole grid);
+    (ii) a phantom that is mirror-symmetric in x and in z (water cylinder, source on the y axis) gives
+        mirror-symmetric collided fluence: mirrored octants visit tiles in the opposite order, so a
+        wrong tile hand-off, flag or index breaks it (north_star check 5 applied to the GPU);
+    (iii) the result does not depend on the hand-off chunk or the number of resident CTAs."""
+    import torch
+    from paper_1811_12391_b200.inputs import phantoms
+    p = _make("config5", n_group=2, n_iter=2)
+    m = p["mesh"]
+    # (i) abdomen phantom: sampled voxels
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    pu = ctx.new_field()
+    ctx.dos_uncollided(p["sources"][0], p["spectrum"], pu)
+    ctx.dos_check()
+    rng = np.random.default_rng(5)
+    in_beam = torch.nonzero(pu[0].reshape(-1) > 0).reshape(-1).cpu().numpy()
+    cells = np.concatenate([rng.choice(in_beam, 4000, replace=False), rng.integers(0, pu[0].numel(), 2000)])
+    ref = orc.uncollided_at(p["mesh"], p["material"], p["sigma_t"], p["sources"][0], p["spectrum"], cells)
+    got = pu.reshape(p["n_group"], -1)[:, torch.from_numpy(cells).to(pu.device)].cpu().numpy()
+    assert_uncollided_parity(got, ref)
+    ctx.close()
+    del pu
+    # (ii) + (iii) symmetric phantom
+    mat = phantoms.cylinder(m["nx"], m["ny"], m["nz"], m["dx"], m["dy"], m["dz"], radius=15.0, inside=1, outside=0)
+    ctx = dos.Context(p["mesh"], mat, p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    pc = ctx.new_field()
+    ctx.dos_uncollided(p["sources"][0], p["spectrum"])
+    ctx.dos_solve(p["n_iter"])
+    ctx.dos_fluence(pc, None)
+    ctx.dos_check()
+    assert torch.isfinite(pc).all()
+    for g in range(p["n_group"]):
+        a = pc[g]
+        peak = a.abs().max().item()
+        assert peak > 0
+        assert (a - a.flip(2)).abs().max().item() <= 2e-5 * peak, "x mirror symmetry"
+        assert (a - a.flip(0)).abs().max().item() <= 2e-5 * peak, "z mirror symmetry"
+    base = pc.clone()
+    ctx.dos_set_option("sweep_chunk", 5)
+    ctx.dos_set_option("sweep_grid", 97)
+    ctx.dos_uncollided(p["sources"][0], p["spectrum"])
+    ctx.dos_solve(p["n_iter"])
+    ctx.dos_fluence(pc, None)
+    ctx.dos_check()
+    for g in range(p["n_group"]):
+        peak = base[g].abs().max().item()
+        assert (pc[g] - base[g]).abs().max().item() <= 2e-5 * peak, "launch-configuration independence"
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------ method properties --
+def test_uncollided_independent_of_quadrature_and_order(dos):
+    """phi_u does not involve S_N or P_L -> bit-identical across them."""
+    a = _make("config2", nx=24, ny=24, nz=8, voxel=1.6, n_group=4, n_iter=1, sn=4, pl=1)
+    b = _make("config2", nx=24, ny=24, nz=8, voxel=1.6, n_group=4, n_iter=1, sn=8, pl=3)
+    ua = dos.run_problem(a)["phi_u"]
+    ub = dos.run_problem(b)["phi_u"]
+    assert np.array_equal(ua, ub)
+
+
+def test_repeatable_and_context_reuse(dos, orc):
+    """A context is reusable for the next source position; a second run of the same position gives the
+    same answer up to the order of the fp32 moment reductions."""
+    p = _make("config4", nx=28, ny=24, nz=8, voxel=1.4, n_group=4, n_iter=3, n_pos=4)
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    first = dos.run_problem(p, source_index=1, ctx=ctx)
+    other = dos.run_problem(p, source_index=2, ctx=ctx)
+    again = dos.run_problem(p, source_index=1, ctx=ctx)
+    assert np.array_equal(first["phi_u"], again["phi_u"])
+    l2, _ = field_errors(again["dose"], first["dose"])
+    assert l2 < 1e-6
+    assert_problem_parity(other, orc.run_problem(p, source_index=2), "reused context")
+    ctx.close()
+
+
+def test_scan_accumulate_and_host_entry_points(dos, orc):
+    """a9: D_scan = sum_p D_p; the *_host entry points copy in/out and synchronise."""
+    p = _make("config4", nx=24, ny=24, nz=8, voxel=1.6, n_group=4, n_iter=3, n_pos=3)
+    ctx = dos.Context(p["mesh"], np.zeros_like(p["material"]), p["sigma_t"], p["sigma_s"], p["kerma"],
+                      p["quadrature"], p["P_L"])
+    ctx.dos_set_material_host(p["material"])          # the grid given to dos_create is replaced
+    h = np.empty(p["material"].shape, dtype=np.float32)
+    ref = np.zeros(p["material"].shape)
+    for n in range(3):
+        ctx.dos_uncollided(p["sources"][n], p["spectrum"])
+        ctx.dos_solve(p["n_iter"])
+        ctx.dos_dose_host(h, accumulate=(n > 0))
+        ref += orc.run_problem(p, source_index=n)["dose"]
+    assert_dose_parity(h, ref, "scan dose via dos_dose_host")
+    ctx.close()
+
+
+def test_state_machine_and_device_side_errors(dos):
+    p = _make("config1")
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    d = ctx.new_field(groups=False)
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_solve(2)
+    assert e.value.status == -3
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_dose(d)
+    assert e.value.status == -3
+    ctx.dos_uncollided(p["sources"][0], p["spectrum"])
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_dose(d)
+    assert e.value.status == -3
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_solve(0)
+    assert e.value.status == -1
+    bad = dict(p["sources"][0], pos=(0.5, 0.5, 0.5))           # a voxel centre of the 16^3 1 cm mesh
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_uncollided(bad, p["spectrum"])
+    assert e.value.status == -1
+    ctx.close()
+    # material id >= n_mat is found on the device and reported by dos_check
+    mat = p["material"].copy()
+    mat[3, 4, 5] = 7
+    ctx = dos.Context(p["mesh"], mat, p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    ctx.dos_uncollided(p["sources"][0], p["spectrum"])
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_check()
+    assert e.value.status == -1
+    ctx.close()
+
+
+def test_collided_fraction_rises_towards_low_energy(dos):
+    """the uncollided fluence dominates in the upper energy range."""
+    p = _make("config2", n_iter=6)
+    out = dos.run_problem(p)
+    k, j, i = 8, 32, 32
+    frac = out["phi_u"][:, k, j, i] / out["phi_total"][:, k, j, i]
+    assert frac[0] > frac[-4] and frac[0] > 0.5

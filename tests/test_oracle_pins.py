@@ -224,6 +224,10 @@ def test_uncollided_collimation_and_sn_independence(orc):
     p2 = make_problem("config2", nx=16, ny=16, nz=8, voxel=2.4, n_group=3, sn=8, pl=3)
     phi2 = orc.uncollided(p2["mesh"], p2["material"], p2["sigma_t"], p2["sources"][0], p2["spectrum"])
     assert np.array_equal(phi, phi2)
+    # the sampled-voxel entry point is the same per-voxel routine
+    cells = np.random.default_rng(0).integers(0, phi[0].size, 200)
+    at = orc.uncollided_at(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"], cells)
+    assert np.array_equal(at, phi.reshape(3, -1)[:, cells])
 
 
 # ------------------------------------------------------------------ DD cell closed forms ----------
