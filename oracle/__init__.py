@@ -126,7 +126,7 @@ def sweep(mesh, material, sig_t_g, quad, L, Q, reflective=False, bnd_state=None,
         raise ValueError("reflective sweep needs bnd_state")
     rc = lib().orc_sweep(C.byref(ms), _p(mat), _p(_d(sig_t_g)), C.c_int(n_ang), _p(mu), _p(eta), _p(xi), _p(w),
                          C.c_int(L), _p(Qd), _p(phi), C.c_int(int(reflective)), _p(bnd_state),
-                         C.byref(leak) if want_leakage else None, _p(psi))
+                         C.byref(leak) if want_leakage else None, _p(psi), None)
     if rc:
         raise MemoryError("orc_sweep")
     out = [phi.reshape((M,) + mat.shape)]
@@ -142,9 +142,10 @@ def bnd_state_size(mesh, n_ang):
 
 
 def solve(mesh, material, sigma_t, sigma_s, quad, L, n_iter, source_pos=None, phi_u=None, q_ext=None,
-          reflective=False, want_balance=False):
+          reflective=False, want_balance=False, want_abs=False):
     """Group cascade + source iteration. Returns phi_c moments [G][M][nz][ny][nx] (float64)
-    (and, if want_balance, (leak[G], src_last[G]) of each group's last sweep)."""
+    (and, if want_balance, (leak[G], src_last[G]) of each group's last sweep; if want_abs, the
+    diagnostic sum_n w_n |psi_n| [G][nz][ny][nx] of each group's last sweep)."""
     sig_t, sig_s = _d(sigma_t), _d(sigma_s)
     n_mat, G = sig_t.shape
     n_leg = sig_s.shape[1] - 1
@@ -160,13 +161,16 @@ def solve(mesh, material, sigma_t, sigma_s, quad, L, n_iter, source_pos=None, ph
     pu = _d(phi_u).reshape(G, nv) if phi_u is not None else None
     qe = _d(q_ext).reshape(G, M, nv) if q_ext is not None else None
     pos = _d(source_pos) if source_pos is not None else np.zeros(3)
+    pabs = np.zeros((G, nv)) if want_abs else None
     ms = _mesh(mesh)
     rc = lib().orc_solve(C.byref(ms), _p(mat), C.c_int(n_mat), C.c_int(G), C.c_int(n_leg), C.c_int(L), _p(sig_t),
                          _p(sig_s), C.c_int(n_ang), _p(mu), _p(eta), _p(xi), _p(w), _p(pos), _p(pu), _p(qe),
-                         C.c_int(n_iter), C.c_int(int(reflective)), _p(phi_c), _p(leak), _p(src))
+                         C.c_int(n_iter), C.c_int(int(reflective)), _p(phi_c), _p(leak), _p(src), _p(pabs))
     if rc:
         raise MemoryError("orc_solve")
     phi_c = phi_c.reshape((G, M) + mat.shape)
+    if want_abs:
+        return phi_c, pabs.reshape((G,) + mat.shape)
     return (phi_c, leak, src) if want_balance else phi_c
 
 
@@ -187,10 +191,11 @@ def dose(mesh, material, kerma, phi_u, phi_c_moments, dose_in=None):
 
 def run_problem(p, source_index=0, n_iter=None):
     """Whole path O1-O5 for one source position of a problem dict from inputs.make_problem.
-    Returns dict(phi_u, phi_c (scalar, [G][nz][ny][nx]), phi_total, dose, phi_c_moments)."""
+    Returns dict(phi_u, phi_c (scalar, [G][nz][ny][nx]), phi_total, dose, phi_c_moments, phi_c_abs
+    (sum_n w_n |psi_n| of each group's last sweep: the parity tests' conditioning scale))."""
     src = p["sources"][source_index]
     pu = uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
-    pc = solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"],
-               p["n_iter"] if n_iter is None else n_iter, source_pos=src["pos"], phi_u=pu)
+    pc, pabs = solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"],
+                     p["n_iter"] if n_iter is None else n_iter, source_pos=src["pos"], phi_u=pu, want_abs=True)
     tot, d = dose(p["mesh"], p["material"], p["kerma"], pu, pc)
-    return {"phi_u": pu, "phi_c": pc[:, 0], "phi_total": tot, "dose": d, "phi_c_moments": pc}
+    return {"phi_u": pu, "phi_c": pc[:, 0], "phi_total": tot, "dose": d, "phi_c_moments": pc, "phi_c_abs": pabs}

@@ -343,11 +343,14 @@ static size_t bnd_size(const orc_mesh *ms)
  * reflective != 0: incoming boundary flux of angle n = outgoing flux of its mirror image stored in
  *   bnd_state [n_ang][bnd] by the previous call (lagged); bnd_state is updated. (oracle-only, pin 2)
  * leakage (may be NULL): sum over boundary faces of w_n |Omega_n . n| psi_out A  (oracle-only, pin 3)
- * psi_all (may be NULL): [n_ang][Nv] angular flux at cell centres (for the brute-force pin). */
+ * psi_all (may be NULL): [n_ang][Nv] angular flux at cell centres (for the brute-force pin).
+ * phi_abs (may be NULL): [Nv] sum_n w_n |psi_c,n(c)|, the size of the terms of eq. 3 -- a diagnostic
+ *   for the parity tests (conditioning of phi[00] where angular fluxes of both signs cancel); it does
+ *   not enter any result. */
 int orc_sweep(const orc_mesh *ms, const uint8_t *mat, const double *sig_t_g, int n_ang,
               const double *mu, const double *eta, const double *xi, const double *w, int L,
               const double *Q, double *phi_new, int reflective, double *bnd_state, double *leakage,
-              double *psi_all)
+              double *psi_all, double *phi_abs)
 {
     int nx = ms->nx, ny = ms->ny, nz = ms->nz;
     size_t nv = (size_t)nx * ny * nz, nb = bnd_size(ms);
@@ -397,6 +400,14 @@ int orc_sweep(const orc_mesh *ms, const uint8_t *mat, const double *sig_t_g, int
                 double p = w[n] * psi[(size_t)n * nv + cell];
                 for (int lm = 0; lm < M; ++lm) phi_new[(size_t)lm * nv + cell] += ylm[(size_t)n * M + lm] * p;
             }
+        if (phi_abs) {
+#pragma omp for schedule(static)
+            for (long long cell = 0; cell < (long long)nv; ++cell) {
+                double a = 0.0;
+                for (int n = 0; n < n_ang; ++n) a += w[n] * fabs(psi[(size_t)n * nv + cell]);
+                phi_abs[cell] = a;
+            }
+        }
     }
     if (leakage) {
         double lk = 0.0;
@@ -424,12 +435,12 @@ int orc_sweep(const orc_mesh *ms, const uint8_t *mat, const double *sig_t_g, int
  *   phi^(0) = 0; it = 1..n_iter: Q = Q_fix + sigma_sl^{g->g} phi^(it-1); phi^(it) = Sweep(Q)   (R5)
  * phi_c out [G][M][Nv]. leak out [G] (may be NULL): leakage of the LAST sweep of each group.
  * absorbed-source bookkeeping for the balance pin: src_last [G] (may be NULL) = sum_c V Q[00](c) of
- * the last sweep's source. */
+ * the last sweep's source. phi_abs [G][Nv] (may be NULL): orc_sweep's diagnostic of the last sweep. */
 int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_leg, int L,
               const double *sigma_t, const double *sigma_s, int n_ang, const double *mu,
               const double *eta, const double *xi, const double *w, const double *pos,
               const double *phi_u, const double *q_ext, int n_iter, int reflective, double *phi_c,
-              double *leak, double *src_last)
+              double *leak, double *src_last, double *phi_abs)
 {
     size_t nv = (size_t)ms->nx * ms->ny * ms->nz, nb = bnd_size(ms);
     int M = (L + 1) * (L + 1);
@@ -467,7 +478,8 @@ int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_le
                 }
             int last = (it == n_iter);
             rc = orc_sweep(ms, mat, sig_t_g, n_ang, mu, eta, xi, w, L, q, phi, reflective, bnd,
-                           (leak && last) ? &leak[g] : NULL, NULL);
+                           (leak && last) ? &leak[g] : NULL, NULL,
+                           (phi_abs && last) ? phi_abs + (size_t)g * nv : NULL);
             if (last && src_last) {
                 double s = 0.0;
                 for (size_t c = 0; c < nv; ++c) s += q[c];
