@@ -21,7 +21,10 @@ struct Layout {
 struct dos_ctx {
     dos_mesh mesh;
     int n_mat, G, n_leg, L, M, MP, n_ang, per_oct;
-    int ntj, ntk, n_items, ag, n_grp, chunk, grid;
+    int ntj, ntk, n_items, ag, n_grp, chunk, grid;     // ag/n_grp/chunk/grid: sweep (dos_sweep.cu)
+    int n_aux;                                         // aux warps of the sweep CTA
+    int impl;                                          // 0: dos_sweep.cu, 1: dos_sweep_v1.cu
+    int ag1, n_grp1, chunk1, grid1;                    // the same for the first version
     size_t nv;
     cudaStream_t stream;
     const uint8_t *d_mat;        // current material grid (caller's or the workspace copy)
@@ -94,17 +97,21 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     const size_t nv = (size_t)m->nx * m->ny * m->nz;
     const int MP = dos_mpad(L), per = n_ang / 8;
     const int ntj = (m->ny + DOS_TJ - 1) / DOS_TJ, ntk = (m->nz + DOS_TK - 1) / DOS_TK;
-    const int ag = dos_sweep_angles_per_warp(per, L);
-    const int n_grp = ag ? per / ag : 1;
+    const int ag1 = dos_sweep_v1_angles_per_warp(per, L);
+    const int n_grp1 = ag1 ? per / ag1 : 1;
+    // tile-face buffers: the larger of the two sweep versions' layouts
+    const size_t fy_v1 = (size_t)n_ang * ntj * m->nz * m->nx, fz_v1 = (size_t)n_ang * ntk * m->ny * m->nx;
+    const size_t fy_v2 = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK;
+    const size_t fz_v2 = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TJ;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     l.phi_u = take(sizeof(float) * G * nv);
     l.phi_all = take(sizeof(float) * G * nv * MP);
     l.qfix = take(sizeof(float) * nv * MP);
     l.q = take(sizeof(float) * nv * MP);
-    l.fy = take(sizeof(float) * (size_t)n_ang * ntj * m->nz * m->nx);
-    l.fz = take(sizeof(float) * (size_t)n_ang * ntk * m->ny * m->nx);
-    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * n_grp);
+    l.fy = take(sizeof(float) * (fy_v1 > fy_v2 ? fy_v1 : fy_v2));
+    l.fz = take(sizeof(float) * (fz_v1 > fz_v2 ? fz_v1 : fz_v2));
+    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * n_grp1);
     l.queue = take(sizeof(int) * 4);
     l.items = take(sizeof(int) * (size_t)8 * ntj * ntk);
     l.mat = take(nv);
@@ -135,7 +142,7 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
     if (P_L > DOS_MAX_L) return fail(nullptr, DOS_ERR_UNSUPPORTED, "P_L > 5");
     if (q->n_ang < 8 || q->n_ang % 8 || !q->mu || !q->eta || !q->xi || !q->w)
         return fail(nullptr, DOS_ERR_INVALID_ARG, "n_ang must be a positive multiple of 8");
-    if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L) == 0)
+    if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_v1_angles_per_warp(q->n_ang / 8, P_L) == 0)
         return fail(nullptr, DOS_ERR_UNSUPPORTED, "angles per octant cannot be split over <= 12 warps of <= 4 angles");
     return DOS_OK;
 }
@@ -194,9 +201,14 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->ntj = (mesh->ny + DOS_TJ - 1) / DOS_TJ;
     c->ntk = (mesh->nz + DOS_TK - 1) / DOS_TK;
     c->n_items = 8 * c->ntj * c->ntk;
-    c->ag = dos_sweep_angles_per_warp(per, L);
+    c->impl = 0;
+    c->ag = dos_sweep_angles_per_warp(per, L, 0);
     c->n_grp = per / c->ag;
-    c->chunk = mesh->nx <= 64 ? 8 : 16;
+    c->n_aux = dos_sweep_aux_warps(per, L, c->ag, 0);
+    c->chunk = 4;
+    c->ag1 = dos_sweep_v1_angles_per_warp(per, L);
+    c->n_grp1 = per / c->ag1;
+    c->chunk1 = mesh->nx <= 64 ? 8 : 16;
     c->nv = (size_t)mesh->nx * mesh->ny * mesh->nz;
     c->stream = (cudaStream_t)cuda_stream;
     c->d_mat = d_material_ids;
@@ -262,7 +274,8 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     if (e == cudaSuccess) e = up(lay.items, items.data(), sizeof(int) * items.size());
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.errflag, 0, sizeof(int) * 4, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // host vectors go out of scope
-    if (e == cudaSuccess) e = dos_sweep_grid(L, c->ag, per, n_mat, c->n_items, &c->grid);
+    if (e == cudaSuccess) e = dos_sweep_grid(L, c->ag, c->n_aux, per, n_mat, c->n_items, &c->grid);
+    if (e == cudaSuccess) e = dos_sweep_v1_grid(L, c->ag1, per, n_mat, c->n_items, &c->grid1);
     if (e != cudaSuccess) {
         std::string msg = std::string("dos_create: ") + cudaGetErrorString(e);
         delete c;
@@ -391,29 +404,36 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
     int *done = (int *)(c->ws + c->lay.done), *queue = (int *)(c->ws + c->lay.queue);
     const MeshDev md = mesh_dev(c->mesh);
     const SourceDev sd = source_dev(c->src);
-    SweepArgs a;
-    a.nx = c->mesh.nx; a.ny = c->mesh.ny; a.nz = c->mesh.nz;
-    a.ntj = c->ntj; a.ntk = c->ntk; a.n_items = c->n_items; a.per_oct = c->per_oct; a.n_grp = c->n_grp;
-    a.chunk = c->chunk; a.n_mat = c->n_mat;
-    a.items = (const int *)(c->ws + c->lay.items);
-    a.Q = q; a.mat = c->d_mat;
-    a.m2d = (const float *)(c->ws + c->lay.m2d); a.d2m = (const float *)(c->ws + c->lay.d2m);
-    a.cdd = (const float *)(c->ws + c->lay.cdd);
-    a.fy = (float *)(c->ws + c->lay.fy); a.fz = (float *)(c->ws + c->lay.fz);
-    a.done = done; a.queue = queue;
-    a.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
+    SweepArgs a1;                       // first version (option sweep_impl = 1)
+    a1.nx = c->mesh.nx; a1.ny = c->mesh.ny; a1.nz = c->mesh.nz;
+    a1.ntj = c->ntj; a1.ntk = c->ntk; a1.n_items = c->n_items; a1.per_oct = c->per_oct; a1.n_grp = c->n_grp1;
+    a1.chunk = c->chunk1; a1.n_mat = c->n_mat;
+    a1.items = (const int *)(c->ws + c->lay.items);
+    a1.Q = q; a1.mat = c->d_mat;
+    a1.m2d = (const float *)(c->ws + c->lay.m2d); a1.d2m = (const float *)(c->ws + c->lay.d2m);
+    a1.cdd = (const float *)(c->ws + c->lay.cdd);
+    a1.fy = (float *)(c->ws + c->lay.fy); a1.fz = (float *)(c->ws + c->lay.fz);
+    a1.done = done; a1.queue = queue;
+    a1.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
+    Sweep2Args a;
+    a.nx = a1.nx; a.ny = a1.ny; a.nz = a1.nz; a.ntj = a1.ntj; a.ntk = a1.ntk; a.n_items = a1.n_items;
+    a.per_oct = a1.per_oct; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = a1.n_mat;
+    a.items = a1.items; a.Q = q; a.mat = c->d_mat; a.m2d = a1.m2d; a.d2m = a1.d2m; a.cdd = a1.cdd;
+    a.fy = a1.fy; a.fz = a1.fz; a.done = done; a.queue = queue; a.abort_flag = a1.abort_flag;
+    const int n_flags = c->impl == 1 ? c->n_items * c->n_grp1 : c->n_items;
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
         CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
                                             phi_all, qfix, c->stream));
         c->launches += 1;
-        a.phi = phi;
-        a.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
+        a.phi = a1.phi = phi;
+        a.sig_t = a1.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
         for (int it = 0; it < n_iter; ++it) {
             CUDA_TRY(c, dos_launch_source_update(c->nv, c->d_mat, c->G, c->n_leg, c->L, g, sig_s, qfix, phi, q, it == 0,
-                                                 done, c->n_items * c->n_grp, queue, c->stream));
+                                                 done, n_flags, queue, c->stream));
             prof_begin(c, 0);
-            CUDA_TRY(c, dos_launch_sweep(a, c->L, c->ag, c->grid, c->stream));
+            if (c->impl == 1) CUDA_TRY(c, dos_launch_sweep_v1(a1, c->L, c->ag1, c->grid1, c->stream));
+            else CUDA_TRY(c, dos_launch_sweep(a, c->L, c->ag, c->grid, c->stream));
             prof_end(c);
             c->launches += 2;
         }
@@ -475,12 +495,28 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
     if (!c || !name) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
     if (!strcmp(name, "sweep_chunk")) {
         if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_chunk must be >= 1");
-        c->chunk = (int)value;
+        c->chunk = c->chunk1 = (int)value;
+    } else if (!strcmp(name, "sweep_impl")) {
+        if (value != 0 && value != 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_impl must be 0 or 1");
+        c->impl = (int)value;
+    } else if (!strcmp(name, "sweep_angles_per_warp")) {
+        const int ag = dos_sweep_angles_per_warp(c->per_oct, c->L, (int)value);
+        if (ag != (int)value) return fail(c, DOS_ERR_INVALID_ARG, "sweep_angles_per_warp: not admissible for this quadrature");
+        const int nx = dos_sweep_aux_warps(c->per_oct, c->L, ag, 0);
+        int grid = 0;
+        CUDA_TRY(c, dos_sweep_grid(c->L, ag, nx, c->per_oct, c->n_mat, c->n_items, &grid));
+        c->ag = ag; c->n_grp = c->per_oct / ag; c->n_aux = nx; c->grid = grid;
+    } else if (!strcmp(name, "sweep_aux_warps")) {
+        const int nx = dos_sweep_aux_warps(c->per_oct, c->L, c->ag, (int)value);
+        if (value < 1 || c->n_grp + nx + 1 > 24) return fail(c, DOS_ERR_INVALID_ARG, "sweep_aux_warps: not admissible");
+        int grid = 0;
+        CUDA_TRY(c, dos_sweep_grid(c->L, c->ag, nx, c->per_oct, c->n_mat, c->n_items, &grid));
+        c->n_aux = nx; c->grid = grid;
     } else if (!strcmp(name, "profile")) {
         c->profile = value != 0;
     } else if (!strcmp(name, "sweep_grid")) {
         if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_grid must be >= 1");
-        c->grid = (int)(value < c->n_items ? value : c->n_items);
+        c->grid = c->grid1 = (int)(value < c->n_items ? value : c->n_items);
     } else {
         return fail(c, DOS_ERR_INVALID_ARG, std::string("unknown option ") + name);
     }

@@ -38,7 +38,44 @@ struct SweepArgs {
     int *abort_flag;         // set by the watchdog; every waiting warp then stops waiting
 };
 
-// dos_sweep.cu
-cudaError_t dos_launch_sweep(const SweepArgs &a, int L, int ang_per_warp, int grid, cudaStream_t s);
-int dos_sweep_angles_per_warp(int per_oct, int L);
-cudaError_t dos_sweep_grid(int L, int ang_per_warp, int per_oct, int n_mat, int n_items, int *grid_out);
+// dos_sweep_v1.cu (first version; option sweep_impl=1)
+cudaError_t dos_launch_sweep_v1(const SweepArgs &a, int L, int ang_per_warp, int grid, cudaStream_t s);
+int dos_sweep_v1_angles_per_warp(int per_oct, int L);
+cudaError_t dos_sweep_v1_grid(int L, int ang_per_warp, int per_oct, int n_mat, int n_items, int *grid_out);
+
+// ---- dos_sweep.cu: the sweep the library uses by default ----
+#define DOS_FACE_PAD 8      // diagonal index d = x + (lane offset) runs over [0, nx + DOS_FACE_PAD)
+#define DOS_PREFETCH_Q 6    // steps between issuing the cp.async of a step's source moments and using them
+#define DOS_RING_Q 8
+#define DOS_PREFETCH_F 3    // the same for tile-inflow faces
+#define DOS_RING_F 4
+
+// Arguments of one launch (all 8 octants, one energy group, one source iteration).
+struct Sweep2Args {
+    int nx, ny, nz;
+    int ntj, ntk;            // tiles along j and k
+    int n_items;             // 8 * ntj * ntk work items (octant, tile)
+    int per_oct;             // angles per octant (A)
+    int n_warps;             // compute warps per CTA (A / AG)
+    int n_aux;               // aux warps per CTA (staging + D2M); the CTA has one more (service) warp
+    int chunk;               // steps between flag publications
+    int n_mat;
+    const int *items;        // [n_items] packed (octant | tj << 3 | tk << 17), dependency-safe order
+    const float *Q;          // [Nv][MP] frozen source moments
+    float *phi;              // [Nv][MP] accumulates w Y psi (zeroed before the launch)
+    const uint8_t *mat;      // [Nv]
+    const float *sig_t;      // [n_mat] total cross section of this group
+    const float *m2d;        // [8][A][MP] (2l+1) Y_lm(Omega_n)
+    const float *d2m;        // [8][A][MP] w_n Y_lm(Omega_n)
+    const float *cdd;        // [A][4] cx, cy, cz, cx+cy+cz
+    float *fy;               // [n_items (by id)][nx + PAD][A][TK] y-face fluxes leaving a tile, by diagonal
+    float *fz;               // [n_items (by id)][nx + PAD][A][TJ] z-face fluxes leaving a tile, by diagonal
+    int *done;               // [n_items (by id)] steps finished and published
+    int *queue;              // work-queue head
+    int *abort_flag;         // set by the watchdog; every waiting CTA then stops waiting
+};
+
+cudaError_t dos_launch_sweep(const Sweep2Args &a, int L, int ang_per_warp, int grid, cudaStream_t s);
+int dos_sweep_angles_per_warp(int per_oct, int L, int prefer);
+cudaError_t dos_sweep_grid(int L, int ang_per_warp, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out);
+int dos_sweep_aux_warps(int per_oct, int L, int ang_per_warp, int prefer);

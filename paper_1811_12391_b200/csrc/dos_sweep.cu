@@ -1,29 +1,89 @@
 // dos_sweep.cu -- the S_N transport sweep (eq. 2-3) for one group and one source
-// iteration: moment-to-discrete, diamond-difference cell update with set-to-zero fixup (north_star;
-// DESIGN.md readings R3, R11, R12), discrete-to-moment, all 8 octants in one launch.
+// iteration: moment-to-discrete (a5), diamond-difference cell update with set-to-zero fixup and
+// rebalance (a6; north_star; readings R3, R11, R12), discrete-to-moment (a7), all 8 octants
+// in one launch. DESIGN.md section 6 has the mapping and the measurements behind it.
 //
-// Mapping:
-//   work item   = (octant, tile of 8 x 4 (j,k) columns), whole x range; items are taken from a queue in
-//                 an order in which every item's upwind neighbours come earlier (tile diagonal major)
-//   CTA         = one item at a time; its warps split the octant's angles (AG angles per warp)
-//   lane        = one (j,k) column of the tile; it marches along x with its x-face flux in a register.
-//                 Lane (jj,kk) is jj+kk cells behind lane (0,0), so the y/z-face fluxes it needs were
-//                 produced one step earlier by lanes (jj-1,kk) / (jj,kk-1): warp shuffles, no barrier.
-//   tile faces  = y/z-face fluxes crossing a tile boundary go through an L2-resident buffer, published
-//                 every `chunk` cells with a release flag that the downwind item's warp polls.
-//   moments     = each lane reads its cell's Q[lm] (float4s, prefetched one step ahead) and adds its
-//                 angles' w Y psi with one vector reduction (red.global.add.v4.f32) per 4 moments.
-// The angular flux psi never leaves registers.
+//   work item   (octant, tile of 8 x 4 (j,k) columns), whole x range. Items sit in a queue in an order
+//               in which an item's two upwind tiles come earlier (tile-diagonal major); persistent
+//               CTAs pop them.
+//   CTA         all A angles of the octant for one tile: NW = A / AG compute warps (AG angles each)
+//               plus one service warp that only polls and publishes hand-off flags.
+//   lane        one (j,k) column; it marches along x with its x-face flux in a register. Lane (jj,kk)
+//               is jj+kk cells behind lane (0,0) (KBA wavefront inside the warp), so the y/z-face
+//               fluxes it needs left lanes (jj-1,kk) / (jj,kk-1) one step earlier: warp shuffles.
+//   step        one x-advance of the whole CTA, closed by one __syncthreads.
+//   staging     the step's 32 source-moment vectors Q[cell][MP] and its tile-inflow face fluxes are
+//               copied into a shared-memory ring by cp.async DOS_PREFETCH steps ahead (one 16-byte
+//               copy per thread per step), so no warp waits on L2/HBM inside a step.
+//   moments     every warp leaves psi_c in shared memory; after the barrier the cell's w Y psi is
+//               summed over ALL angles of the octant by (cell, 4-moment) threads and added to
+//               phi[cell][lm] with one red.global.add.v4.f32 per cell, octant and 4 moments (the first
+//               version issued one per warp: A/AG times as many).
+//   tile faces  fluxes crossing a tile boundary go through an L2-resident buffer indexed by the
+//               wavefront diagonal (d = x + kk for y faces, x + jj for z faces), so what a downwind
+//               step needs is one contiguous block; published every `chunk` steps with a release
+//               store that the downwind CTA's service warp acquires.
+// The angular flux psi never leaves registers / shared memory.
 #include "dos_internal.h"
 
 namespace {
 
-__device__ __forceinline__ int ld_acquire(const int *p)
+constexpr int DQ = DOS_PREFETCH_Q;    // steps between issuing the copy of a step's source moments and using them
+constexpr int RQ = DOS_RING_Q;        // ring slots of the staged moments (power of two > DQ)
+constexpr int DF = DOS_PREFETCH_F;    // the same for the tile-inflow faces (shorter: it delays a downwind tile's start)
+constexpr int RF = DOS_RING_F;
+constexpr int BIG = 1 << 30;
+constexpr int FINW = DOS_TK + DOS_TJ;   // inflow floats per angle and step: 4 y faces then 8 z faces
+
+__device__ __forceinline__ int ld_relaxed(const int *p)
 {
     int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+
+// CTA-scope release / acquire on a shared-memory word (service warp <-> compute warps)
+__device__ __forceinline__ void st_release_cta(int *p, int v)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ int ld_acquire_cta(const int *p)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+
+// shared-memory accesses through explicit 32-bit shared addresses (keeps the address arithmetic of the
+// step loop to one integer add per access)
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float lds_f32(unsigned a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ int lds_s32(unsigned a)
+{
+    int v;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float4 lds_v4(unsigned a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_f32(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts_s32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+
+// barrier of the compute warps only (the service warp never joins it)
+__device__ __forceinline__ void bar_compute(int n_threads) { asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory"); }
 
 __device__ __forceinline__ void st_release(int *p, int v)
 {
@@ -37,210 +97,412 @@ __device__ __forceinline__ void red_add_v4(float *p, float4 v)
                  : "memory");
 }
 
-// Diamond-difference cell update with set-to-zero fixup and rebalance. pin/pout: x, y, z faces.
-__device__ __forceinline__ float dd_update(float q, float st, float cx, float cy, float cz, float cs, float ix,
-                                           float iy, float iz, float &ox, float &oy, float &oz)
+// 16-byte asynchronous global -> shared copy that bypasses L1 (tile faces are written by other SMs
+// during this launch; an L1 line could be stale)
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
-    float num = fmaf(cx, ix, fmaf(cy, iy, fmaf(cz, iz, q)));
-    float pc = num / (st + cs);
-    ox = 2.f * pc - ix;
-    oy = 2.f * pc - iy;
-    oz = 2.f * pc - iz;
-    if (ox < 0.f || oy < 0.f || oz < 0.f) {
-        bool fx = false, fy = false, fz = false;
-        for (;;) {
-            bool ax = !fx && ox < 0.f, ay = !fy && oy < 0.f, az = !fz && oz < 0.f;
-            if (!(ax || ay || az)) break;
-            fx |= ax; fy |= ay; fz |= az;
-            num = q + (fx ? 0.5f * cx : cx) * ix + (fy ? 0.5f * cy : cy) * iy + (fz ? 0.5f * cz : cz) * iz;
-            float den = st + (fx ? 0.f : cx) + (fy ? 0.f : cy) + (fz ? 0.f : cz);
-            pc = num / den;
-            ox = fx ? 0.f : 2.f * pc - ix;
-            oy = fy ? 0.f : 2.f * pc - iy;
-            oz = fz ? 0.f : 2.f * pc - iz;
-        }
-    }
-    return pc;
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-template <int MP, int AG>
-__global__ void __launch_bounds__(384) sweep_kernel(const SweepArgs p)
-{
-    constexpr int MV = MP / 4;
-    extern __shared__ float4 smem4[];
-    float *s_m2d = reinterpret_cast<float *>(smem4);      // [A][MP] for the current octant
-    float *s_d2m = s_m2d + p.per_oct * MP;                 // [A][MP]
-    float *s_cdd = s_d2m + p.per_oct * MP;                 // [A][4]
-    float *s_sig = s_cdd + p.per_oct * 4;                  // [n_mat]
-    __shared__ int s_item;
+// shared-memory row length of one cell's moments: MP floats, padded so that MPS/4 is odd and the
+// per-lane LDS.128 of a warp (lane stride MPS floats) are bank-conflict free
+__host__ __device__ constexpr int mps_of(int MP) { return ((MP / 4) & 1) ? MP : MP + 4; }
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+// Slow path of the cell update: at least one extrapolated outflow was negative. Faces found negative
+// are pinned to zero together, the balance is re-solved, and the pinned set only grows (R12).
+// in/out: o = (psi_c, out_x, out_y, out_z) of the unfixed solve -> of the fixed one.
+__device__ __noinline__ float4 dd_fixup(float4 o, float q, float st, float cx, float cy, float cz, float ix, float iy,
+                                        float iz)
+{
+    bool fx = false, fy = false, fz = false;
+    for (;;) {
+        const bool ax = !fx && o.y < 0.f, ay = !fy && o.z < 0.f, az = !fz && o.w < 0.f;
+        if (!(ax || ay || az)) break;
+        fx |= ax; fy |= ay; fz |= az;
+        const float num = q + (fx ? 0.5f * cx : cx) * ix + (fy ? 0.5f * cy : cy) * iy + (fz ? 0.5f * cz : cz) * iz;
+        const float den = st + (fx ? 0.f : cx) + (fy ? 0.f : cy) + (fz ? 0.f : cz);
+        o.x = num / den;
+        o.y = fx ? 0.f : 2.f * o.x - ix;
+        o.z = fy ? 0.f : 2.f * o.x - iy;
+        o.w = fz ? 0.f : 2.f * o.x - iz;
+    }
+    return o;
+}
+
+// One cp.async of 16 bytes that a thread issues every step: at step t it fetches what step s = t + dist
+// needs (if s lies inside the window [lo, hi]) from src0 + s * sstep (floats) into ring slot s & mask.
+struct LoadOp {
+    const float *src0;
+    float *dst0;
+    int sstep, dslot, lo, hi, dist, mask;
+};
+
+struct ItemGeom {
+    int o, tj, tk, id;
+    bool has_y, has_z;
+    const float *fy_in, *fz_in;
+};
+
+// Decode load `op` of the current item: ops [0, 32 MV) fetch 4 moments of lane c's cell, the next A
+// fetch the 4 y-face inflows of angle a, the last 2A the 8 z-face inflows of angle a in two halves.
+template <int MP>
+__device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const ItemGeom &g, float *s_q, float *s_fin)
+{
+    constexpr int MV = MP / 4, MPS = mps_of(MP);
+    const int A = p.per_oct, nx = p.nx;
+    LoadOp d;
+    d.lo = 1; d.hi = 0;                      // empty window
+    d.src0 = p.Q; d.dst0 = s_q; d.sstep = 0; d.dslot = 0; d.dist = DQ; d.mask = RQ - 1;
+    if (op < 32 * MV) {
+        const int c = op / MV, v = op - c * MV;
+        const int jj = c & (DOS_TJ - 1), kk = c / DOS_TJ, skew = jj + kk;
+        const int jp = g.tj * DOS_TJ + jj, kp = g.tk * DOS_TK + kk;
+        if (jp < p.ny && kp < p.nz) {
+            const int j = (g.o & 2) ? p.ny - 1 - jp : jp, k = (g.o & 4) ? p.nz - 1 - kp : kp;
+            const int istep = (g.o & 1) ? -1 : 1;
+            const long long cell0 = ((long long)k * p.ny + j) * nx + ((g.o & 1) ? nx - 1 : 0);
+            d.sstep = istep * MP;
+            d.src0 = p.Q + (cell0 - (long long)istep * skew) * MP + 4 * v;
+            d.lo = skew; d.hi = skew + nx - 1;
+        }
+        d.dst0 = s_q + c * MPS + 4 * v;
+        d.dslot = 32 * MPS;
+    } else if (op < 32 * MV + A) {
+        const int a = op - 32 * MV;
+        if (g.has_y) { d.lo = 0; d.hi = nx + DOS_TK - 2; }
+        d.src0 = g.fy_in + a * DOS_TK;
+        d.sstep = A * DOS_TK;
+        d.dst0 = s_fin + a * FINW;
+        d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
+    } else {
+        const int idx = op - 32 * MV - A, a = idx >> 1, h = idx & 1;
+        if (g.has_z) { d.lo = 0; d.hi = nx + DOS_TJ - 2; }
+        d.src0 = g.fz_in + a * DOS_TJ + 4 * h;
+        d.sstep = A * DOS_TJ;
+        d.dst0 = s_fin + a * FINW + DOS_TK + 4 * h;
+        d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
+    }
+    return d;
+}
+
+// Warp roles inside a CTA (one work item at a time):
+//   compute warps  [0, NW)        AG angles each: M2D, diamond difference, face hand-off, psi_c to smem
+//   aux warps      [NW, NW + NX)  staging copies (cp.async), material ids, D2M reduction + red.global of
+//                                 the previous step, progress counter
+//   service warp   NW + NX        global hand-off flags (never joins the per-step barrier)
+// TMAX = CTA size bound for the register budget.
+template <int MP, int AG, int TMAX>
+__global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
+{
+    constexpr int MV = MP / 4, MPS = mps_of(MP);
+    extern __shared__ float4 smem4[];
+    const int A = p.per_oct, NW = p.n_warps, NX = p.n_aux;
+    const int NB = (NW + NX) * 32;                          // threads in the per-step barrier
+    float *s_q = reinterpret_cast<float *>(smem4);          // [RQ][32][MPS] staged source moments
+    float *s_fin = s_q + RQ * 32 * MPS;                     // [RF][A][FINW] staged tile-inflow faces
+    float *s_psi = s_fin + RF * A * FINW;                   // [2][A][32]    psi_c of the last two steps
+    float *s_m2d = s_psi + 2 * A * 32;                      // [A][MP] for the current octant
+    float *s_d2m = s_m2d + A * MP;                          // [A][MP]
+    float *s_cdd = s_d2m + A * MP;                          // [A][4]
+    float *s_rden = s_cdd + A * 4;                          // [n_mat][A]  1 / (sigma_t + cx + cy + cz)
+    float *s_sig = s_rden + p.n_mat * A;                    // [n_mat]
+    int *s_mat = reinterpret_cast<int *>(s_sig + ((p.n_mat + 3) & ~3));   // [4][32] material ids of 4 steps
+    __shared__ int s_item;
+    __shared__ int s_done;        // steps finished by the compute/aux warps (written by one aux thread)
+    __shared__ int s_allowed;     // last step whose tile-inflow faces are published upwind (service warp)
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool service = warp == NW + NX, aux = warp >= NW && !service;
     const int jj = lane & (DOS_TJ - 1), kk = lane / DOS_TJ;
     const int skew = jj + kk;
-    const int nx = p.nx, ny = p.ny, nz = p.nz, A = p.per_oct;
-    const int a0 = warp * AG;
+    const int nx = p.nx, ny = p.ny, nz = p.nz;
+    const int T = nx + DOS_SKEW;
+    const size_t fstride_y = (size_t)(nx + DOS_FACE_PAD) * A * DOS_TK, fstride_z = (size_t)(nx + DOS_FACE_PAD) * A * DOS_TJ;
 
-    for (int t = threadIdx.x; t < A * 4; t += blockDim.x) s_cdd[t] = p.cdd[t];
-    for (int t = threadIdx.x; t < p.n_mat; t += blockDim.x) s_sig[t] = p.sig_t[t];
+    for (int t = tid; t < A * 4; t += blockDim.x) s_cdd[t] = p.cdd[t];
+    for (int t = tid; t < p.n_mat; t += blockDim.x) s_sig[t] = p.sig_t[t];
+    for (int t = tid; t < p.n_mat * A; t += blockDim.x) {
+        const int m = t / A, a = t - m * A;
+        s_rden[t] = 1.f / (p.sig_t[m] + p.cdd[a * 4 + 3]);
+    }
     int cur_oct = -1;
 
     for (;;) {
-        __syncthreads();
-        if (threadIdx.x == 0) s_item = atomicAdd(p.queue, 1);
+        __syncthreads();                              // previous item finished with the staging buffers
+        if (tid == 0) s_item = atomicAdd(p.queue, 1);
         __syncthreads();
         const int item = s_item;
         if (item >= p.n_items) break;
         const int packed = p.items[item];
-        const int o = packed & 7, tj = (packed >> 3) & 0x3FFF, tk = packed >> 17;
+        ItemGeom g;
+        g.o = packed & 7; g.tj = (packed >> 3) & 0x3FFF; g.tk = packed >> 17;
+        g.id = (g.o * p.ntk + g.tk) * p.ntj + g.tj;
+        g.has_y = g.tj > 0; g.has_z = g.tk > 0;
+        g.fy_in = p.fy + (g.has_y ? (size_t)(g.id - 1) * fstride_y : 0);
+        g.fz_in = p.fz + (g.has_z ? (size_t)(g.id - p.ntj) * fstride_z : 0);
+        const int o = g.o;
         if (o != cur_oct) {
-            for (int t = threadIdx.x; t < A * MP; t += blockDim.x) {
+            for (int t = tid; t < A * MP; t += blockDim.x) {
                 s_m2d[t] = p.m2d[(size_t)o * A * MP + t];
                 s_d2m[t] = p.d2m[(size_t)o * A * MP + t];
             }
             cur_oct = o;
-            __syncthreads();
         }
 
-        // ---- per-lane geometry of this item (oriented indices: primes sweep upwards) ----
-        const int jp = tj * DOS_TJ + jj, kp = tk * DOS_TK + kk;
+        if (service) {
+            // ------- service warp: publishes this item's progress, follows the upwind items' progress -------
+            // It never joins the per-step barrier, so the latency of its global loads, fences and stores
+            // stays off the other warps' critical path; the two sides talk through s_done / s_allowed.
+            const int *up_y = p.done + (g.has_y ? g.id - 1 : g.id), *up_z = p.done + (g.has_z ? g.id - p.ntj : g.id);
+            int *my_flag = p.done + g.id;
+            int avail_y = g.has_y ? 0 : BIG, avail_z = g.has_z ? 0 : BIG;
+            if (lane == 0) {
+                s_done = 0;
+                s_allowed = (g.has_y || g.has_z) ? -1 : BIG;
+            }
+            __syncthreads();                          // S2
+            int published = 0, spins = 0;
+            for (;;) {
+                const int dn = ld_acquire_cta(&s_done);
+                if (dn - published >= p.chunk || (dn == T && published < T)) {
+                    if (lane == 0) st_release(my_flag, dn);       // steps < dn are complete
+                    published = dn;
+                }
+                if (published == T) break;
+                if (avail_y < T || avail_z < T) {
+                    const int vy = avail_y < T ? ld_relaxed(up_y) : avail_y;
+                    const int vz = avail_z < T ? ld_relaxed(up_z) : avail_z;
+                    if (vy != avail_y || vz != avail_z) {
+                        fence_acq_rel_gpu();          // relaxed load + fence = acquire of the upwind release
+                        avail_y = vy; avail_z = vz;
+                        const int al = min(avail_y >= T ? BIG : avail_y - DOS_TJ, avail_z >= T ? BIG : avail_z - DOS_TK);
+                        if (lane == 0) st_release_cta(&s_allowed, al);
+                        spins = 0;
+                    } else {
+                        // watchdog: a hand-off that never arrives must not hang the GPU; the result is then
+                        // invalid and dos_check / dos_dose_host report DOS_ERR_CUDA
+                        if (++spins > DOS_SPIN_LIMIT) atomicExch(p.abort_flag, 1);
+                        if ((spins & 255) == 0 && ld_relaxed(p.abort_flag)) {
+                            avail_y = avail_z = BIG;
+                            if (lane == 0) st_release_cta(&s_allowed, BIG);
+                        }
+                        __nanosleep(64);
+                    }
+                } else {
+                    __nanosleep(128);
+                }
+            }
+            continue;
+        }
+
+        // geometry of this lane's (j,k) column: its cell at step t is cbase + istep * t, for t - t_lo in [0, nx)
+        const int jp = g.tj * DOS_TJ + jj, kp = g.tk * DOS_TK + kk;
         const bool valid = jp < ny && kp < nz;
         const int j = (o & 2) ? ny - 1 - jp : jp;
         const int k = (o & 4) ? nz - 1 - kp : kp;
         const int istep = (o & 1) ? -1 : 1;
-        const size_t cell0 = ((size_t)k * ny + j) * nx + ((o & 1) ? nx - 1 : 0);
-        const bool load_y = valid && jj == 0 && tj > 0;
-        const bool load_z = valid && kk == 0 && tk > 0;
-        const bool store_y = valid && jj == DOS_TJ - 1 && tj < p.ntj - 1;
-        const bool store_z = valid && kk == DOS_TK - 1 && tk < p.ntk - 1;
-        const size_t ystride = (size_t)p.ntj * nz * nx, zstride = (size_t)p.ntk * ny * nx;
-        const float *fy_in = p.fy + (((size_t)(o * A + a0) * p.ntj + (tj - 1)) * nz + kp) * nx;
-        float *fy_out = p.fy + (((size_t)(o * A + a0) * p.ntj + tj) * nz + kp) * nx;
-        const float *fz_in = p.fz + (((size_t)(o * A + a0) * p.ntk + (tk - 1)) * ny + jp) * nx;
-        float *fz_out = p.fz + (((size_t)(o * A + a0) * p.ntk + tk) * ny + jp) * nx;
-        const int id = (o * p.ntk + tk) * p.ntj + tj;
-        int *my_flag = p.done + (size_t)id * p.n_grp + warp;
-        const int *up_y = p.done + (size_t)(id - 1) * p.n_grp + warp;
-        const int *up_z = p.done + (size_t)(id - p.ntj) * p.n_grp + warp;
-        const bool dep_y = tj > 0, dep_z = tk > 0;
-        int avail = (dep_y || dep_z) ? 0 : nx;    // cells along x whose upwind tile faces are published
+        const long long cbase = ((long long)k * ny + j) * nx + ((o & 1) ? nx - 1 : 0) - (long long)istep * skew;
+        const int t_lo = valid ? skew : BIG;
 
+        if (aux) {
+            // ---------------- aux warps: staging, material ids, D2M of the previous step ----------------
+            const int xw = warp - NW, xt = tid - NW * 32, NXT = NX * 32;
+            const int n_ops = 32 * MV + 3 * A;
+            const LoadOp op0 = make_op<MP>(xt, p, g, s_q, s_fin);
+            const LoadOp op1 = make_op<MP>(xt + NXT < n_ops ? xt + NXT : xt, p, g, s_q, s_fin);
+            const bool op0_on = xt < n_ops, op1_on = xt + NXT < n_ops, more_ops = n_ops > 2 * NXT;
+            const uint8_t *mat_p = p.mat + cbase + 3 * istep;            // material of step t + 3
+            float *phi_p = p.phi + (cbase - istep) * MP;                 // moments of the cell of step t - 1
+            const int phi_inc = istep * MP;
+            const unsigned psi_r = smem_addr(s_psi + lane), d2m_a = smem_addr(s_d2m);
+            const unsigned mat_w = smem_addr(s_mat + lane);
+            const int psi_slot = A * 32 * 4;
+            auto mat_of = [&](int s, const uint8_t *q) -> int {
+                return ((unsigned)(s - t_lo) < (unsigned)nx) ? (int)__ldg(q) : 0;
+            };
+            __syncthreads();                          // S2: octant tables, s_done, s_allowed in place
+            int allowed_c = -1;
+            auto gate = [&](int s) {                  // wait until the upwind tiles have published step s
+                while (allowed_c < s) {
+                    allowed_c = ld_acquire_cta(&s_allowed);
+                    if (allowed_c < s) __nanosleep(64);
+                }
+            };
+            auto issue_one = [&](const LoadOp &d, int tau) {
+                const int s = tau + d.dist;
+                if (s >= d.lo && s <= d.hi) {
+                    if (d.dist == DF) gate(s);
+                    cp_async16(d.dst0 + (s & d.mask) * d.dslot, d.src0 + (long long)s * d.sstep);
+                }
+            };
+            // round tau fetches the moments of step tau + DQ and the tile-inflow faces of step tau + DF
+            auto issue_round = [&](int tau) {
+                if (op0_on) issue_one(op0, tau);
+                if (op1_on) issue_one(op1, tau);
+                if (more_ops)
+                    for (int op = xt + 2 * NXT; op < n_ops; op += NXT) issue_one(make_op<MP>(op, p, g, s_q, s_fin), tau);
+                cp_async_commit();
+            };
+            for (int tau = -DQ; tau < 0; ++tau) issue_round(tau);
+            int reg_m = 0;
+            if (xw == 0) {
+                sts_s32(mat_w, mat_of(0, mat_p - 3 * istep));
+                sts_s32(mat_w + 128, mat_of(1, mat_p - 2 * istep));
+                reg_m = mat_of(2, mat_p - istep);
+            }
+            cp_async_wait<DF - 1>();
+            bar_compute(NB);                          // S3: step 0's staged data visible to every warp
+
+#pragma unroll 1
+            for (int t = 0; t < T; ++t) {
+                issue_round(t);
+                if (xw == 0) {
+                    sts_s32(mat_w + ((t + 2) & 3) * 128, reg_m);
+                    reg_m = mat_of(t + 3, mat_p);
+                    mat_p += istep;
+                }
+                // D2M of step t - 1: sum over all angles of the octant, one red per (cell, 4 moments)
+                if (t > 0 && (unsigned)(t - 1 - t_lo) < (unsigned)nx) {
+                    const unsigned ps = psi_r + ((t - 1) & 1) * psi_slot;
+                    for (int v = xw; v < MV; v += NX) {
+                        const unsigned dp = d2m_a + 16 * v;
+                        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 5
+                        for (int a = 0; a < A; ++a) {
+                            const float psi = lds_f32(ps + a * 128);
+                            const float4 d = lds_v4(dp + a * (MP * 4));
+                            acc.x = fmaf(d.x, psi, acc.x);
+                            acc.y = fmaf(d.y, psi, acc.y);
+                            acc.z = fmaf(d.z, psi, acc.z);
+                            acc.w = fmaf(d.w, psi, acc.w);
+                        }
+                        red_add_v4(phi_p + 4 * v, acc);
+                    }
+                }
+                phi_p += phi_inc;
+                cp_async_wait<DF - 1>();              // step t + 1's staged data complete (this thread's copies)
+                bar_compute(NB);                      // B_t: ... and visible to all
+                if (xt == 0) st_release_cta(&s_done, t + 1);
+            }
+            if ((unsigned)(T - 1 - t_lo) < (unsigned)nx) {
+                const unsigned ps = psi_r + ((T - 1) & 1) * psi_slot;
+                for (int v = xw; v < MV; v += NX) {
+                    const unsigned dp = d2m_a + 16 * v;
+                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int a = 0; a < A; ++a) {
+                        const float psi = lds_f32(ps + a * 128);
+                        const float4 d = lds_v4(dp + a * (MP * 4));
+                        acc.x = fmaf(d.x, psi, acc.x);
+                        acc.y = fmaf(d.y, psi, acc.y);
+                        acc.z = fmaf(d.z, psi, acc.z);
+                        acc.w = fmaf(d.w, psi, acc.w);
+                    }
+                    red_add_v4(phi_p + 4 * v, acc);
+                }
+            }
+            continue;
+        }
+
+        // ---------------- compute warps: M2D, diamond difference, face hand-off ----------------
+        constexpr bool REGC = AG * MP <= 48;          // M2D coefficients of this warp's angles in registers
+        const int a0 = warp * AG;
+        const bool in_y = jj == 0, in_z = kk == 0;
+        const bool has_y = g.has_y, has_z = g.has_z;
+        const bool store_y = valid && jj == DOS_TJ - 1 && g.tj < p.ntj - 1;
+        const bool store_z = valid && kk == DOS_TK - 1 && g.tk < p.ntk - 1;
+        // running pointers, advanced once per step
+        float *fy_st = p.fy + (size_t)g.id * fstride_y + kk + ((long long)(1 - DOS_TJ) * A + a0) * DOS_TK;
+        float *fz_st = p.fz + (size_t)g.id * fstride_z + jj + ((long long)(1 - DOS_TK) * A + a0) * DOS_TJ;
+        const int fy_inc = A * DOS_TK, fz_inc = A * DOS_TJ;
+        const unsigned fin_y = smem_addr(s_fin + a0 * FINW + kk), fin_z = smem_addr(s_fin + a0 * FINW + DOS_TK + jj);
+        const unsigned psi_w = smem_addr(s_psi + a0 * 32 + lane);
+        const unsigned q_row = smem_addr(s_q + lane * MPS);
+        const unsigned rden_a = smem_addr(s_rden + a0), sig_a = smem_addr(s_sig), mat_r = smem_addr(s_mat + lane);
+        const unsigned m2d_a = smem_addr(s_m2d + a0 * MP);
+        const int fin_slot = A * FINW * 4, psi_slot = A * 32 * 4, A4 = A * 4;
+
+        float cm[REGC ? AG * MP : 1];
+        float ccx[AG], ccy[AG], ccz[AG];
+        __syncthreads();                              // S2: octant tables, s_done, s_allowed in place
+        if (REGC) {
+#pragma unroll
+            for (int r = 0; r < AG; ++r)
+#pragma unroll
+                for (int e = 0; e < MP; ++e) cm[REGC ? r * MP + e : 0] = s_m2d[(a0 + r) * MP + e];
+        }
+#pragma unroll
+        for (int r = 0; r < AG; ++r) {
+            ccx[r] = s_cdd[(a0 + r) * 4 + 0]; ccy[r] = s_cdd[(a0 + r) * 4 + 1]; ccz[r] = s_cdd[(a0 + r) * 4 + 2];
+        }
         float px[AG], oy[AG], oz[AG];
 #pragma unroll
         for (int r = 0; r < AG; ++r) px[r] = oy[r] = oz[r] = 0.f;
+        bar_compute(NB);                              // S3: step 0's staged data visible
 
-        float4 qn[MV];
-        float byn[AG], bzn[AG];
-        int matn = 0;
+#pragma unroll 1
+        for (int t = 0; t < T; ++t) {
+            // moment-to-discrete for this lane's cell, AG angles; four partial sums keep the FMA chains short
+            const bool act = (unsigned)(t - t_lo) < (unsigned)nx;
+            const int m0 = lds_s32(mat_r + (t & 3) * 128);
+            float q[AG];
+            {
+                float part[AG][4];
 #pragma unroll
-        for (int v = 0; v < MV; ++v) qn[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int r = 0; r < AG; ++r) part[r][0] = part[r][1] = part[r][2] = part[r][3] = 0.f;
+                const unsigned qs = q_row + (t & (RQ - 1)) * (32 * MPS * 4);
 #pragma unroll
-        for (int r = 0; r < AG; ++r) byn[r] = bzn[r] = 0.f;
-
-        const int T = nx + DOS_SKEW;
-        for (int t = -1; t < T; ++t) {
-            // ---- rotate the prefetched operands of step t into place ----
-            float4 qc[MV];
-            float byc[AG], bzc[AG];
+                for (int v = 0; v < MV; ++v) {
+                    const float4 qv = lds_v4(qs + 16 * v);
 #pragma unroll
-            for (int v = 0; v < MV; ++v) qc[v] = qn[v];
-#pragma unroll
-            for (int r = 0; r < AG; ++r) { byc[r] = byn[r]; bzc[r] = bzn[r]; }
-            const int matc = matn;
-
-            // ---- prefetch step t+1 (needs the upwind faces of cell t+1 of the lead lane) ----
-            if (t + 1 < T) {
-                const int need = min(t + 2, nx);
-                int spins = 0;
-                while (avail < need) {
-                    int ya = dep_y ? ld_acquire(up_y) : nx;
-                    int za = dep_z ? ld_acquire(up_z) : nx;
-                    avail = min(ya, za);
-                    if (avail < need) {
-                        __nanosleep(40);
-                        // watchdog: a hand-off that never arrives must not hang the GPU; the result is
-                        // then invalid and dos_check / dos_dose_host report DOS_ERR_CUDA
-                        if (++spins > DOS_SPIN_LIMIT) atomicExch(p.abort_flag, 1);
-                        if ((spins & 255) == 0 && ld_acquire(p.abort_flag)) avail = nx;
+                    for (int r = 0; r < AG; ++r) {
+                        float4 c;
+                        if (REGC) c = make_float4(cm[REGC ? r * MP + 4 * v : 0], cm[REGC ? r * MP + 4 * v + 1 : 0],
+                                                  cm[REGC ? r * MP + 4 * v + 2 : 0], cm[REGC ? r * MP + 4 * v + 3 : 0]);
+                        else c = lds_v4(m2d_a + (r * MP + 4 * v) * 4);
+                        part[r][v & 3] = fmaf(c.x, qv.x, fmaf(c.y, qv.y, fmaf(c.z, qv.z, fmaf(c.w, qv.w, part[r][v & 3]))));
                     }
                 }
-                const int ipn = t + 1 - skew;
-                if (valid && ipn >= 0 && ipn < nx) {
-                    const size_t cell = cell0 + (ptrdiff_t)istep * ipn;
-                    const float4 *qp = reinterpret_cast<const float4 *>(p.Q) + cell * MV;
 #pragma unroll
-                    for (int v = 0; v < MV; ++v) qn[v] = __ldg(qp + v);
-                    matn = __ldg(p.mat + cell);
-                    if (load_y) {
-#pragma unroll
-                        for (int r = 0; r < AG; ++r) byn[r] = __ldcg(fy_in + r * ystride + ipn);
-                    }
-                    if (load_z) {
-#pragma unroll
-                        for (int r = 0; r < AG; ++r) bzn[r] = __ldcg(fz_in + r * zstride + ipn);
-                    }
-                }
+                for (int r = 0; r < AG; ++r) q[r] = (part[r][0] + part[r][1]) + (part[r][2] + part[r][3]);
             }
-            if (t < 0) continue;
 
-            // ---- step t: this lane's cell is ip = t - skew ----
-            const int ip = t - skew;
-            const bool act = valid && ip >= 0 && ip < nx;
-            float yin[AG], zin[AG];
+            // inflow, diamond difference, outflow
+            const unsigned fslot = (t & (RF - 1)) * fin_slot;
+            const unsigned pso = psi_w + (t & 1) * psi_slot;
+            const unsigned rd = rden_a + m0 * A4;
+            const bool first_x = t == t_lo;
 #pragma unroll
             for (int r = 0; r < AG; ++r) {
-                yin[r] = __shfl_up_sync(0xffffffffu, oy[r], 1);
-                zin[r] = __shfl_up_sync(0xffffffffu, oz[r], DOS_TJ);
-                if (jj == 0) yin[r] = load_y ? byc[r] : 0.f;     // tile inflow or vacuum
-                if (kk == 0) zin[r] = load_z ? bzc[r] : 0.f;
-            }
-            if (act) {
-                const size_t cell = cell0 + (ptrdiff_t)istep * ip;
-                const float st = s_sig[matc];
-                float q[AG], pc[AG];
-#pragma unroll
-                for (int r = 0; r < AG; ++r) q[r] = 0.f;
-#pragma unroll
-                for (int v = 0; v < MV; ++v) {
-#pragma unroll
-                    for (int r = 0; r < AG; ++r) {
-                        const float4 c = *reinterpret_cast<const float4 *>(s_m2d + (a0 + r) * MP + 4 * v);
-                        q[r] = fmaf(c.x, qc[v].x, fmaf(c.y, qc[v].y, fmaf(c.z, qc[v].z, fmaf(c.w, qc[v].w, q[r]))));
+                float yin = __shfl_up_sync(0xffffffffu, oy[r], 1);
+                float zin = __shfl_up_sync(0xffffffffu, oz[r], DOS_TJ);
+                if (in_y) yin = has_y ? lds_f32(fin_y + fslot + r * (FINW * 4)) : 0.f;    // tile inflow or vacuum
+                if (in_z) zin = has_z ? lds_f32(fin_z + fslot + r * (FINW * 4)) : 0.f;
+                float pc = 0.f;
+                if (act) {
+                    const float ix = first_x ? 0.f : px[r];
+                    const float num = fmaf(ccx[r], ix, fmaf(ccy[r], yin, fmaf(ccz[r], zin, q[r])));
+                    pc = num * lds_f32(rd + 4 * r);
+                    float ox = 2.f * pc - ix, oyr = 2.f * pc - yin, ozr = 2.f * pc - zin;
+                    if (fminf(ox, fminf(oyr, ozr)) < 0.f) {
+                        const float4 f = dd_fixup(make_float4(pc, ox, oyr, ozr), q[r], lds_f32(sig_a + 4 * m0), ccx[r], ccy[r],
+                                                  ccz[r], ix, yin, zin);
+                        pc = f.x; ox = f.y; oyr = f.z; ozr = f.w;
                     }
-                }
-#pragma unroll
-                for (int r = 0; r < AG; ++r) {
-                    const float4 c = *reinterpret_cast<const float4 *>(s_cdd + (a0 + r) * 4);
-                    const float ix = (ip == 0) ? 0.f : px[r];
-                    float ox, oyr, ozr;
-                    pc[r] = dd_update(q[r], st, c.x, c.y, c.z, c.w, ix, yin[r], zin[r], ox, oyr, ozr);
                     px[r] = ox; oy[r] = oyr; oz[r] = ozr;
-                    if (store_y) __stcg(fy_out + r * ystride + ip, oyr);
-                    if (store_z) __stcg(fz_out + r * zstride + ip, ozr);
+                    if (store_y) __stcg(fy_st + r * DOS_TK, oyr);
+                    if (store_z) __stcg(fz_st + r * DOS_TJ, ozr);
                 }
-                float *php = p.phi + cell * MP;
-#pragma unroll
-                for (int v = 0; v < MV; ++v) {
-                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                    for (int r = 0; r < AG; ++r) {
-                        const float4 d = *reinterpret_cast<const float4 *>(s_d2m + (a0 + r) * MP + 4 * v);
-                        acc.x = fmaf(d.x, pc[r], acc.x);
-                        acc.y = fmaf(d.y, pc[r], acc.y);
-                        acc.z = fmaf(d.z, pc[r], acc.z);
-                        acc.w = fmaf(d.w, pc[r], acc.w);
-                    }
-                    red_add_v4(php + 4 * v, acc);
-                }
+                sts_f32(pso + r * 128, pc);
             }
-            // ---- publish: the slowest lane (skew DOS_SKEW) has just finished cell t - DOS_SKEW ----
-            const int fin = t - DOS_SKEW;
-            if (fin >= 0 && (((fin + 1) % p.chunk) == 0 || fin == nx - 1)) {
-                __syncwarp();
-                if (lane == 0) {
-                    __threadfence();
-                    st_release(my_flag, fin + 1);
-                }
-            }
+            fy_st += fy_inc; fz_st += fz_inc;
+            bar_compute(NB);                          // B_t
         }
     }
 }
@@ -250,51 +512,71 @@ __global__ void __launch_bounds__(384) sweep_kernel(const SweepArgs p)
 // ------------------------------------------------------------------------------------------------
 // host side: choice of angles per warp, occupancy-sized persistent grid, template dispatch
 // ------------------------------------------------------------------------------------------------
-typedef void (*sweep_fn)(const SweepArgs);
+typedef void (*sweep_fn)(const Sweep2Args);
 
 template <int MP>
-static sweep_fn pick_ag(int ag)
+static sweep_fn pick_ag(int ag, bool big)
 {
     switch (ag) {
-        case 1: return sweep_kernel<MP, 1>;
-        case 2: return sweep_kernel<MP, 2>;
-        case 3: return sweep_kernel<MP, 3>;
-        case 4: return sweep_kernel<MP, 4>;
+        case 1: return big ? sweep_kernel<MP, 1, 768> : sweep_kernel<MP, 1, 512>;
+        case 2: return big ? sweep_kernel<MP, 2, 768> : sweep_kernel<MP, 2, 512>;
+        case 3: return big ? sweep_kernel<MP, 3, 768> : sweep_kernel<MP, 3, 512>;
+        case 4: return big ? sweep_kernel<MP, 4, 768> : sweep_kernel<MP, 4, 512>;
     }
     return nullptr;
 }
 
-static sweep_fn pick(int L, int ag)
+// CTAs of more than 16 warps (compute + aux + service) need the 768-thread variant
+static sweep_fn pick(int L, int ag, int per_oct, int n_aux)
 {
+    const bool big = per_oct / ag + n_aux + 1 > 16;
     switch (dos_mpad(L)) {
-        case 4: return pick_ag<4>(ag);
-        case 12: return pick_ag<12>(ag);
-        case 16: return pick_ag<16>(ag);
-        case 28: return pick_ag<28>(ag);
-        case 36: return pick_ag<36>(ag);
+        case 4: return pick_ag<4>(ag, big);
+        case 12: return pick_ag<12>(ag, big);
+        case 16: return pick_ag<16>(ag, big);
+        case 28: return pick_ag<28>(ag, big);
+        case 36: return pick_ag<36>(ag, big);
     }
     return nullptr;
 }
 
 static size_t sweep_smem(int L, int per_oct, int n_mat)
 {
-    return sizeof(float) * ((size_t)2 * per_oct * dos_mpad(L) + 4 * per_oct + n_mat + 4);
+    const int MP = dos_mpad(L), MPS = mps_of(MP), A = per_oct;
+    const size_t floats = (size_t)RQ * 32 * MPS + (size_t)RF * A * FINW + (size_t)2 * A * 32 + (size_t)2 * A * MP +
+                          (size_t)4 * A + (size_t)n_mat * A + ((n_mat + 3) & ~3) + 4 * 32 + 4;
+    return sizeof(float) * floats;
 }
 
-// Angles per warp: the largest of 4, 3, 2, 1 that divides the octant's angle count and keeps the CTA
-// within 12 warps (S2: 1x1, S4: 3 -> 1 warp, S6: 6 -> 3x2, S8: 10 -> 5x2, S12: 21 -> 7x3, S16: 36 -> 9x4).
-int dos_sweep_angles_per_warp(int per_oct, int L)
+// Angles per warp AG (1..4, must divide the octant's angle count A; the CTA has A/AG compute warps and
+// one service warp, at most 21 warps). Default: the smallest AG with at most 12 compute warps -- few
+// angles per warp keep the per-step dependent chain short (S2: 1x1, S4: 3x1, S6: 6x1, S8: 10x1,
+// S12: 7x3, S16: 12x3). `prefer` > 0 overrides when it is admissible.
+// Aux warps (staging + D2M): one per 4-moment quad when the CTA then stays within 16 warps, else fewer
+// (each takes several quads). `prefer` > 0 overrides (clamped to [1, MP/4]).
+int dos_sweep_aux_warps(int per_oct, int L, int ag, int prefer)
+{
+    const int mv = dos_mpad(L) / 4, nw = per_oct / ag;
+    if (prefer >= 1) return prefer < mv ? prefer : mv;
+    int nx = mv;
+    while (nx > 1 && nw + nx + 1 > 16) nx = (nx + 1) / 2;
+    return nx;
+}
+
+int dos_sweep_angles_per_warp(int per_oct, int L, int prefer)
 {
     (void)L;
-    int best = 0;
-    for (int ag = 4; ag >= 1; --ag)
-        if (per_oct % ag == 0 && per_oct / ag <= 12) { best = ag; break; }
-    return best;
+    if (prefer >= 1 && prefer <= 4 && per_oct % prefer == 0 && per_oct / prefer <= (prefer <= 2 ? 20 : 12)) return prefer;
+    for (int ag = 1; ag <= 4; ++ag)
+        if (per_oct % ag == 0 && per_oct / ag <= 12) return ag;
+    for (int ag = 1; ag <= 2; ++ag)
+        if (per_oct % ag == 0 && per_oct / ag <= 20) return ag;
+    return 0;
 }
 
-cudaError_t dos_sweep_grid(int L, int ag, int per_oct, int n_mat, int n_items, int *grid_out)
+cudaError_t dos_sweep_grid(int L, int ag, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out)
 {
-    sweep_fn f = pick(L, ag);
+    sweep_fn f = pick(L, ag, per_oct, n_aux);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, per_oct, n_mat);
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -302,7 +584,7 @@ cudaError_t dos_sweep_grid(int L, int ag, int per_oct, int n_mat, int n_items, i
     int dev = 0, sms = 0, per_sm = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    const int threads = (per_oct / ag) * 32;
+    const int threads = (per_oct / ag + n_aux + 1) * 32;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, threads, smem)) != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     // Persistent CTAs: every resident CTA pulls items until the queue is empty. All CTAs of the grid
@@ -312,11 +594,11 @@ cudaError_t dos_sweep_grid(int L, int ag, int per_oct, int n_mat, int n_items, i
     return cudaSuccess;
 }
 
-cudaError_t dos_launch_sweep(const SweepArgs &a, int L, int ag, int grid, cudaStream_t s)
+cudaError_t dos_launch_sweep(const Sweep2Args &a, int L, int ag, int grid, cudaStream_t s)
 {
-    sweep_fn f = pick(L, ag);
+    sweep_fn f = pick(L, ag, a.per_oct, a.n_aux);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, a.per_oct, a.n_mat);
-    f<<<grid, a.n_grp * 32, smem, s>>>(a);
+    f<<<grid, (a.n_warps + a.n_aux + 1) * 32, smem, s>>>(a);
     return cudaGetLastError();
 }
