@@ -508,7 +508,7 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
         c->ag = ag; c->n_grp = c->per_oct / ag; c->n_aux = nx; c->grid = grid;
     } else if (!strcmp(name, "sweep_aux_warps")) {
         const int nx = dos_sweep_aux_warps(c->per_oct, c->L, c->ag, (int)value);
-        if (value < 1 || c->n_grp + nx + 1 > 24) return fail(c, DOS_ERR_INVALID_ARG, "sweep_aux_warps: not admissible");
+        if (value < 1 || c->n_grp + nx + 2 > 24) return fail(c, DOS_ERR_INVALID_ARG, "sweep_aux_warps: not admissible");
         int grid = 0;
         CUDA_TRY(c, dos_sweep_grid(c->L, c->ag, nx, c->per_oct, c->n_mat, c->n_items, &grid));
         c->n_aux = nx; c->grid = grid;

@@ -196,7 +196,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
 //   compute warps  [0, NW)        AG angles each: M2D, diamond difference, face hand-off, psi_c to smem
 //   aux warps      [NW, NW + NX)  staging copies (cp.async), material ids, D2M reduction + red.global of
 //                                 the previous step, progress counter
-//   service warp   NW + NX        global hand-off flags (never joins the per-step barrier)
+//   tick warp      NW + NX        joins the per-step barrier only to publish the step count to the service warp
+//   service warp   NW + NX + 1    global hand-off flags (never joins the per-step barrier)
 // TMAX = CTA size bound for the register budget.
 template <int MP, int AG, int TMAX>
 __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
@@ -204,7 +205,7 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
     constexpr int MV = MP / 4, MPS = mps_of(MP);
     extern __shared__ float4 smem4[];
     const int A = p.per_oct, NW = p.n_warps, NX = p.n_aux;
-    const int NB = (NW + NX) * 32;                          // threads in the per-step barrier
+    const int NB = (NW + NX + 1) * 32;                      // threads in the per-step barrier (compute, aux, tick)
     float *s_q = reinterpret_cast<float *>(smem4);          // [RQ][32][MPS] staged source moments
     float *s_fin = s_q + RQ * 32 * MPS;                     // [RF][A][FINW] staged tile-inflow faces
     float *s_psi = s_fin + RF * A * FINW;                   // [2][A][32]    psi_c of the last two steps
@@ -219,7 +220,7 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
     __shared__ int s_allowed;     // last step whose tile-inflow faces are published upwind (service warp)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const bool service = warp == NW + NX, aux = warp >= NW && !service;
+    const bool tick = warp == NW + NX, service = warp == NW + NX + 1, aux = warp >= NW && warp < NW + NX;
     const int jj = lane & (DOS_TJ - 1), kk = lane / DOS_TJ;
     const int skew = jj + kk;
     const int nx = p.nx, ny = p.ny, nz = p.nz;
@@ -298,6 +299,20 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
                 } else {
                     __nanosleep(128);
                 }
+            }
+            continue;
+        }
+
+        if (tick) {
+            // ------- tick warp: counts the per-step barriers for the service warp -------
+            // It has no global memory traffic of its own, so its CTA-scope release costs nothing, while the
+            // same release issued by an aux or compute thread would wait for that warp's outstanding
+            // red.global / st.global round trips to L2 on every step.
+            __syncthreads();                          // S2
+            bar_compute(NB);                          // S3
+            for (int t = 0; t < T; ++t) {
+                bar_compute(NB);                      // B_t: every face store of step t precedes it
+                if (lane == 0) st_release_cta(&s_done, t + 1);
             }
             continue;
         }
@@ -389,7 +404,6 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
                 phi_p += phi_inc;
                 cp_async_wait<DF - 1>();              // step t + 1's staged data complete (this thread's copies)
                 bar_compute(NB);                      // B_t: ... and visible to all
-                if (xt == 0) st_release_cta(&s_done, t + 1);
             }
             if ((unsigned)(T - 1 - t_lo) < (unsigned)nx) {
                 const unsigned ps = psi_r + ((T - 1) & 1) * psi_slot;
@@ -529,7 +543,7 @@ static sweep_fn pick_ag(int ag, bool big)
 // CTAs of more than 16 warps (compute + aux + service) need the 768-thread variant
 static sweep_fn pick(int L, int ag, int per_oct, int n_aux)
 {
-    const bool big = per_oct / ag + n_aux + 1 > 16;
+    const bool big = per_oct / ag + n_aux + 2 > 16;
     switch (dos_mpad(L)) {
         case 4: return pick_ag<4>(ag, big);
         case 12: return pick_ag<12>(ag, big);
@@ -552,14 +566,14 @@ static size_t sweep_smem(int L, int per_oct, int n_mat)
 // one service warp, at most 21 warps). Default: the smallest AG with at most 12 compute warps -- few
 // angles per warp keep the per-step dependent chain short (S2: 1x1, S4: 3x1, S6: 6x1, S8: 10x1,
 // S12: 7x3, S16: 12x3). `prefer` > 0 overrides when it is admissible.
-// Aux warps (staging + D2M): one per 4-moment quad when the CTA then stays within 16 warps, else fewer
+// Aux warps (staging + D2M): one per 4-moment quad when the CTA then stays within 24 warps, else fewer
 // (each takes several quads). `prefer` > 0 overrides (clamped to [1, MP/4]).
 int dos_sweep_aux_warps(int per_oct, int L, int ag, int prefer)
 {
     const int mv = dos_mpad(L) / 4, nw = per_oct / ag;
     if (prefer >= 1) return prefer < mv ? prefer : mv;
     int nx = mv;
-    while (nx > 1 && nw + nx + 1 > 16) nx = (nx + 1) / 2;
+    while (nx > 1 && nw + nx + 2 > 24) nx = (nx + 1) / 2;
     return nx;
 }
 
@@ -584,7 +598,7 @@ cudaError_t dos_sweep_grid(int L, int ag, int n_aux, int per_oct, int n_mat, int
     int dev = 0, sms = 0, per_sm = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    const int threads = (per_oct / ag + n_aux + 1) * 32;
+    const int threads = (per_oct / ag + n_aux + 2) * 32;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f, threads, smem)) != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     // Persistent CTAs: every resident CTA pulls items until the queue is empty. All CTAs of the grid
@@ -599,6 +613,6 @@ cudaError_t dos_launch_sweep(const Sweep2Args &a, int L, int ag, int grid, cudaS
     sweep_fn f = pick(L, ag, a.per_oct, a.n_aux);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, a.per_oct, a.n_mat);
-    f<<<grid, (a.n_warps + a.n_aux + 1) * 32, smem, s>>>(a);
+    f<<<grid, (a.n_warps + a.n_aux + 2) * 32, smem, s>>>(a);
     return cudaGetLastError();
 }
