@@ -137,7 +137,12 @@ dos_status dos_dose_host(dos_ctx *ctx, float *h_dose, int32_t accumulate);
 dos_status dos_check(dos_ctx *ctx);
 
 /* Tuning / measurement knobs (all optional).
- *   "sweep_chunk"   cells along x between face-flux hand-offs of neighbouring tiles (>= 1)
+ *   "sweep_chunk"   steps along x between face-flux hand-off publications of neighbouring tiles (>= 1)
+ *   "sweep_grid"    number of persistent sweep CTAs
+ *   "sweep_angles_per_warp", "sweep_aux_warps", "sweep_angle_split"  shape of the sweep CTA and number of
+ *                   CTAs an octant's angles are spread over (0 = library default)
+ *   "sweep_impl"    0: dos_sweep.cu (default), 1: the first version kept for A/B measurements
+ *   "sweep_trace_item"  see dos_sweep_trace_host
  *   "profile"       1: bracket every sweep and ray-trace launch with CUDA events (see dos_profile)  */
 dos_status dos_set_option(dos_ctx *ctx, const char *name, int64_t value);
 
@@ -152,6 +157,14 @@ typedef struct {
 } dos_profile_t;
 dos_status dos_profile(dos_ctx *ctx, dos_profile_t *out);
 dos_status dos_profile_reset(dos_ctx *ctx);
+
+/* Diagnostic timeline of one sweep work item (option "sweep_trace_item" = (octant * ntk + tk) * ntj + tj, -1 =
+ * off): after a dos_solve, copies to HOST the SM clock at which every warp of that item's CTA started each step
+ * (k = 0), finished its first phase (1: staging copies for aux warps, moment-to-discrete for compute warps), its
+ * second phase (2: discrete-to-moment / diamond difference) and reached the step's barrier (3), in the last
+ * sweep launched: h_trace[(step * 32 + warp) * 4 + k], step < nx + 10, n = number of int64 to copy.
+ * Synchronises the stream. */
+dos_status dos_sweep_trace_host(dos_ctx *ctx, int64_t *h_trace, size_t n);
 
 void dos_destroy(dos_ctx *ctx);
 

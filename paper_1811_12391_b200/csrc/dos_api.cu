@@ -15,7 +15,7 @@
 
 struct Layout {
     size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
-        spectrum, errflag, total;
+        spectrum, errflag, trace, total;
 };
 
 struct dos_ctx {
@@ -23,6 +23,8 @@ struct dos_ctx {
     int n_mat, G, n_leg, L, M, MP, n_ang, per_oct;
     int ntj, ntk, n_items, ag, n_grp, chunk, grid;     // ag/n_grp/chunk/grid: sweep (dos_sweep.cu)
     int n_aux;                                         // aux warps of the sweep CTA
+    int asplit, ag_pref, aux_pref;                     // angle split of an octant over CTAs; option overrides (0 = default)
+    int trace_item;                                    // sweep work item whose timeline is recorded, or -1
     int impl;                                          // 0: dos_sweep.cu, 1: dos_sweep_v1.cu
     int ag1, n_grp1, chunk1, grid1;                    // the same for the first version
     size_t nv;
@@ -111,7 +113,7 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.q = take(sizeof(float) * nv * MP);
     l.fy = take(sizeof(float) * (fy_v1 > fy_v2 ? fy_v1 : fy_v2));
     l.fz = take(sizeof(float) * (fz_v1 > fz_v2 ? fz_v1 : fz_v2));
-    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * n_grp1);
+    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * (n_grp1 > 8 ? n_grp1 : 8));   // v2: up to 8 angle parts per tile
     l.queue = take(sizeof(int) * 4);
     l.items = take(sizeof(int) * (size_t)8 * ntj * ntk);
     l.mat = take(nv);
@@ -124,6 +126,7 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.cdd = take(sizeof(float) * per * 4);
     l.spectrum = take(sizeof(double) * G);
     l.errflag = take(sizeof(int) * 4);
+    l.trace = take(sizeof(long long) * (size_t)(m->nx + DOS_SKEW) * 32 * 4);
     l.total = off;
     return l;
 }
@@ -145,6 +148,32 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
     if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_v1_angles_per_warp(q->n_ang / 8, P_L) == 0)
         return fail(nullptr, DOS_ERR_UNSUPPORTED, "angles per octant cannot be split over <= 12 warps of <= 4 angles");
     return DOS_OK;
+}
+
+// Shape of the sweep CTA (dos_sweep.cu) for the current option values: angle split of an octant over CTAs,
+// angles per compute warp, aux warps, persistent grid.
+static cudaError_t configure_sweep(dos_ctx *c)
+{
+    int as = c->asplit;
+    if (as < 1 || c->per_oct % as) as = 1;
+    const int ap = c->per_oct / as;
+    const int ag = dos_sweep_angles_per_warp(ap, c->L, c->ag_pref);
+    if (ag == 0) return cudaErrorInvalidValue;
+    const int nx = dos_sweep_aux_warps(ap, c->L, ag, c->aux_pref);
+    int grid = 0;
+    cudaError_t e = dos_sweep_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, &grid);
+    if (e != cudaSuccess) return e;
+    c->asplit = as; c->ag = ag; c->n_grp = ap / ag; c->n_aux = nx; c->grid = grid;
+    return cudaSuccess;
+}
+
+// Default angle split: one CTA per (octant, tile). Spreading an octant's angles over 2 or more CTAs (option
+// "sweep_angle_split") shortens a step on meshes of a few tiles but replicates the moment staging and the
+// reductions; measured on config 2 it is a wash, so it stays an option.
+static int default_asplit(int per_oct, int n_tiles_items)
+{
+    (void)per_oct; (void)n_tiles_items;
+    return 1;
 }
 
 extern "C" dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs, const dos_quadrature *quad,
@@ -202,9 +231,9 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->ntk = (mesh->nz + DOS_TK - 1) / DOS_TK;
     c->n_items = 8 * c->ntj * c->ntk;
     c->impl = 0;
-    c->ag = dos_sweep_angles_per_warp(per, L, 0);
-    c->n_grp = per / c->ag;
-    c->n_aux = dos_sweep_aux_warps(per, L, c->ag, 0);
+    c->trace_item = -1;
+    c->ag_pref = c->aux_pref = 0;
+    c->asplit = default_asplit(per, c->n_items);
     c->chunk = 4;
     c->ag1 = dos_sweep_v1_angles_per_warp(per, L);
     c->n_grp1 = per / c->ag1;
@@ -274,7 +303,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     if (e == cudaSuccess) e = up(lay.items, items.data(), sizeof(int) * items.size());
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.errflag, 0, sizeof(int) * 4, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // host vectors go out of scope
-    if (e == cudaSuccess) e = dos_sweep_grid(L, c->ag, c->n_aux, per, n_mat, c->n_items, &c->grid);
+    if (e == cudaSuccess) e = configure_sweep(c);
     if (e == cudaSuccess) e = dos_sweep_v1_grid(L, c->ag1, per, n_mat, c->n_items, &c->grid1);
     if (e != cudaSuccess) {
         std::string msg = std::string("dos_create: ") + cudaGetErrorString(e);
@@ -417,10 +446,13 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
     a1.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
     Sweep2Args a;
     a.nx = a1.nx; a.ny = a1.ny; a.nz = a1.nz; a.ntj = a1.ntj; a.ntk = a1.ntk; a.n_items = a1.n_items;
-    a.per_oct = a1.per_oct; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = a1.n_mat;
+    a.per_oct = c->per_oct / c->asplit; a.per_oct_full = c->per_oct; a.a_split = c->asplit;
+    a.n_items = c->n_items * c->asplit; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = a1.n_mat;
     a.items = a1.items; a.Q = q; a.mat = c->d_mat; a.m2d = a1.m2d; a.d2m = a1.d2m; a.cdd = a1.cdd;
     a.fy = a1.fy; a.fz = a1.fz; a.done = done; a.queue = queue; a.abort_flag = a1.abort_flag;
-    const int n_flags = c->impl == 1 ? c->n_items * c->n_grp1 : c->n_items;
+    a.trace = c->trace_item >= 0 ? (long long *)(c->ws + c->lay.trace) : nullptr;
+    a.trace_item = c->trace_item;
+    const int n_flags = c->impl == 1 ? c->n_items * c->n_grp1 : c->n_items * c->asplit;
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
         CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
@@ -499,24 +531,36 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
     } else if (!strcmp(name, "sweep_impl")) {
         if (value != 0 && value != 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_impl must be 0 or 1");
         c->impl = (int)value;
-    } else if (!strcmp(name, "sweep_angles_per_warp")) {
-        const int ag = dos_sweep_angles_per_warp(c->per_oct, c->L, (int)value);
-        if (ag != (int)value) return fail(c, DOS_ERR_INVALID_ARG, "sweep_angles_per_warp: not admissible for this quadrature");
-        const int nx = dos_sweep_aux_warps(c->per_oct, c->L, ag, 0);
-        int grid = 0;
-        CUDA_TRY(c, dos_sweep_grid(c->L, ag, nx, c->per_oct, c->n_mat, c->n_items, &grid));
-        c->ag = ag; c->n_grp = c->per_oct / ag; c->n_aux = nx; c->grid = grid;
-    } else if (!strcmp(name, "sweep_aux_warps")) {
-        const int nx = dos_sweep_aux_warps(c->per_oct, c->L, c->ag, (int)value);
-        if (value < 1 || c->n_grp + nx + 2 > 24) return fail(c, DOS_ERR_INVALID_ARG, "sweep_aux_warps: not admissible");
-        int grid = 0;
-        CUDA_TRY(c, dos_sweep_grid(c->L, c->ag, nx, c->per_oct, c->n_mat, c->n_items, &grid));
-        c->n_aux = nx; c->grid = grid;
+    } else if (!strcmp(name, "sweep_angles_per_warp") || !strcmp(name, "sweep_aux_warps") || !strcmp(name, "sweep_angle_split")) {
+        // 0 = library default
+        const int old_ag = c->ag_pref, old_aux = c->aux_pref, old_as = c->asplit;
+        if (value < 0 || value > 16) return fail(c, DOS_ERR_INVALID_ARG, std::string(name) + " out of range");
+        if (name[6] == 'a' && name[8] == 'g' && name[11] == '_' && name[12] == 's') {     // sweep_angle_split
+            if (value > 8 || (value > 0 && c->per_oct % value)) return fail(c, DOS_ERR_INVALID_ARG, "sweep_angle_split must divide the angles per octant (<= 8)");
+            c->asplit = value > 0 ? (int)value : default_asplit(c->per_oct, c->n_items);
+        } else if (name[7] == 'n') {
+            c->ag_pref = (int)value;
+        } else {
+            c->aux_pref = (int)value;
+        }
+        const bool bad_ag = c->ag_pref > 0 && dos_sweep_angles_per_warp(c->per_oct / c->asplit, c->L, c->ag_pref) != c->ag_pref;
+        cudaError_t e = bad_ag ? cudaErrorInvalidValue : configure_sweep(c);
+        if (e == cudaSuccess && c->n_grp + c->n_aux + 2 > 24) e = cudaErrorInvalidValue;
+        if (e != cudaSuccess) {
+            c->ag_pref = old_ag; c->aux_pref = old_aux; c->asplit = old_as;
+            configure_sweep(c);
+            return fail(c, DOS_ERR_INVALID_ARG, std::string(name) + ": not admissible for this quadrature");
+        }
+    } else if (!strcmp(name, "sweep_trace_item")) {
+        if (value < -1 || value >= c->n_items * c->asplit) return fail(c, DOS_ERR_INVALID_ARG, "sweep_trace_item out of range");
+        c->trace_item = (int)value;
+        CUDA_TRY(c, cudaMemsetAsync(c->ws + c->lay.trace, 0, sizeof(long long) * (size_t)(c->mesh.nx + DOS_SKEW) * 128, c->stream));
     } else if (!strcmp(name, "profile")) {
         c->profile = value != 0;
     } else if (!strcmp(name, "sweep_grid")) {
         if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_grid must be >= 1");
-        c->grid = c->grid1 = (int)(value < c->n_items ? value : c->n_items);
+        c->grid1 = (int)(value < c->n_items ? value : c->n_items);
+        c->grid = (int)(value < c->n_items * c->asplit ? value : c->n_items * c->asplit);
     } else {
         return fail(c, DOS_ERR_INVALID_ARG, std::string("unknown option ") + name);
     }
@@ -531,6 +575,16 @@ extern "C" dos_status dos_profile(dos_ctx *c, dos_profile_t *out)
     out->sweep_ms = c->acc_ms[0]; out->sweep_launches = c->acc_n[0];
     out->raytrace_ms = c->acc_ms[1]; out->raytrace_launches = c->acc_n[1];
     out->kernel_launches = c->launches;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_sweep_trace_host(dos_ctx *c, int64_t *h_trace, size_t n)
+{
+    if (!c || !h_trace) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    const size_t have = (size_t)(c->mesh.nx + DOS_SKEW) * 128;
+    if (n > have) n = have;
+    CUDA_TRY(c, cudaMemcpyAsync(h_trace, c->ws + c->lay.trace, sizeof(int64_t) * n, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return DOS_OK;
 }
 

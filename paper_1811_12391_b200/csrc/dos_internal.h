@@ -54,25 +54,29 @@ cudaError_t dos_sweep_v1_grid(int L, int ang_per_warp, int per_oct, int n_mat, i
 struct Sweep2Args {
     int nx, ny, nz;
     int ntj, ntk;            // tiles along j and k
-    int n_items;             // 8 * ntj * ntk work items (octant, tile)
-    int per_oct;             // angles per octant (A)
+    int n_items;             // 8 * ntj * ntk * a_split work items (octant, tile, angle part); item = tile item * a_split + part
+    int per_oct;             // angles per CTA (A = angles per octant / a_split)
+    int per_oct_full;        // angles per octant
+    int a_split;             // CTAs (angle parts) per (octant, tile)
     int n_warps;             // compute warps per CTA (A / AG)
     int n_aux;               // aux warps per CTA (staging + D2M); the CTA has one more (service) warp
     int chunk;               // steps between flag publications
     int n_mat;
-    const int *items;        // [n_items] packed (octant | tj << 3 | tk << 17), dependency-safe order
+    const int *items;        // [8 * ntj * ntk] packed (octant | tj << 3 | tk << 17), dependency-safe order
     const float *Q;          // [Nv][MP] frozen source moments
     float *phi;              // [Nv][MP] accumulates w Y psi (zeroed before the launch)
     const uint8_t *mat;      // [Nv]
     const float *sig_t;      // [n_mat] total cross section of this group
-    const float *m2d;        // [8][A][MP] (2l+1) Y_lm(Omega_n)
-    const float *d2m;        // [8][A][MP] w_n Y_lm(Omega_n)
-    const float *cdd;        // [A][4] cx, cy, cz, cx+cy+cz
+    const float *m2d;        // [8][per_oct_full][MP] (2l+1) Y_lm(Omega_n)
+    const float *d2m;        // [8][per_oct_full][MP] w_n Y_lm(Omega_n)
+    const float *cdd;        // [per_oct_full][4] cx, cy, cz, cx+cy+cz
     float *fy;               // [n_items (by id)][nx + PAD][A][TK] y-face fluxes leaving a tile, by diagonal
     float *fz;               // [n_items (by id)][nx + PAD][A][TJ] z-face fluxes leaving a tile, by diagonal
     int *done;               // [n_items (by id)] steps finished and published
     int *queue;              // work-queue head
     int *abort_flag;         // set by the watchdog; every waiting CTA then stops waiting
+    long long *trace;        // optional [nx + DOS_SKEW][32][4] SM-clock timeline of item `trace_item` (or null)
+    int trace_item;
 };
 
 cudaError_t dos_launch_sweep(const Sweep2Args &a, int L, int ang_per_warp, int grid, cudaStream_t s);

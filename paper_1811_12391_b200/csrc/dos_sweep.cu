@@ -82,6 +82,14 @@ __device__ __forceinline__ float4 lds_v4(unsigned a)
 __device__ __forceinline__ void sts_f32(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void sts_s32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
+// Optional per-step timeline of one work item (option "sweep_trace_item"): every warp's lane 0 stores the SM
+// clock when it starts a step (0), after its staging / M2D phase (1), after its D2M / diamond-difference phase (2)
+// and when it reaches the step's barrier (3): trace[(step * 32 + warp) * 4 + k].
+__device__ __forceinline__ void trace_mark(long long *trace, int step, int warp, int which)
+{
+    if (trace && (threadIdx.x & 31) == 0) trace[(step * 32 + warp) * 4 + which] = clock64();
+}
+
 // barrier of the compute warps only (the service warp never joins it)
 __device__ __forceinline__ void bar_compute(int n_threads) { asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory"); }
 
@@ -194,9 +202,10 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
 
 // Warp roles inside a CTA (one work item at a time):
 //   compute warps  [0, NW)        AG angles each: M2D, diamond difference, face hand-off, psi_c to smem
-//   aux warps      [NW, NW + NX)  staging copies (cp.async), material ids, D2M reduction + red.global of
-//                                 the previous step, progress counter
-//   tick warp      NW + NX        joins the per-step barrier only to publish the step count to the service warp
+//   aux warps      [NW, NW + NX)  staging copies of the source moments (cp.async), D2M reduction + red.global
+//                                 of the previous step
+//   feeder warp    NW + NX        staging copies of the tile-inflow faces, material ids, step count for the
+//                                 service warp
 //   service warp   NW + NX + 1    global hand-off flags (never joins the per-step barrier)
 // TMAX = CTA size bound for the register budget.
 template <int MP, int AG, int TMAX>
@@ -227,12 +236,7 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
     const int T = nx + DOS_SKEW;
     const size_t fstride_y = (size_t)(nx + DOS_FACE_PAD) * A * DOS_TK, fstride_z = (size_t)(nx + DOS_FACE_PAD) * A * DOS_TJ;
 
-    for (int t = tid; t < A * 4; t += blockDim.x) s_cdd[t] = p.cdd[t];
     for (int t = tid; t < p.n_mat; t += blockDim.x) s_sig[t] = p.sig_t[t];
-    for (int t = tid; t < p.n_mat * A; t += blockDim.x) {
-        const int m = t / A, a = t - m * A;
-        s_rden[t] = 1.f / (p.sig_t[m] + p.cdd[a * 4 + 3]);
-    }
     int cur_oct = -1;
 
     for (;;) {
@@ -241,27 +245,36 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
         __syncthreads();
         const int item = s_item;
         if (item >= p.n_items) break;
-        const int packed = p.items[item];
+        const int tile_item = item / p.a_split, part = item - tile_item * p.a_split;
+        const int packed = p.items[tile_item];
         ItemGeom g;
         g.o = packed & 7; g.tj = (packed >> 3) & 0x3FFF; g.tk = packed >> 17;
-        g.id = (g.o * p.ntk + g.tk) * p.ntj + g.tj;
+        g.id = ((g.o * p.ntk + g.tk) * p.ntj + g.tj) * p.a_split + part;
         g.has_y = g.tj > 0; g.has_z = g.tk > 0;
-        g.fy_in = p.fy + (g.has_y ? (size_t)(g.id - 1) * fstride_y : 0);
-        g.fz_in = p.fz + (g.has_z ? (size_t)(g.id - p.ntj) * fstride_z : 0);
+        g.fy_in = p.fy + (g.has_y ? (size_t)(g.id - p.a_split) * fstride_y : 0);
+        g.fz_in = p.fz + (g.has_z ? (size_t)(g.id - p.ntj * p.a_split) * fstride_z : 0);
         const int o = g.o;
-        if (o != cur_oct) {
+        long long *const trace = (p.trace && g.id == p.trace_item) ? p.trace : nullptr;
+        if (o * 8 + part != cur_oct) {
+            // tables of this CTA's angles: [o][part * A, (part + 1) * A)
+            const size_t abase = (size_t)o * p.per_oct_full + (size_t)part * A;
             for (int t = tid; t < A * MP; t += blockDim.x) {
-                s_m2d[t] = p.m2d[(size_t)o * A * MP + t];
-                s_d2m[t] = p.d2m[(size_t)o * A * MP + t];
+                s_m2d[t] = p.m2d[abase * MP + t];
+                s_d2m[t] = p.d2m[abase * MP + t];
             }
-            cur_oct = o;
+            for (int t = tid; t < A * 4; t += blockDim.x) s_cdd[t] = p.cdd[part * A * 4 + t];
+            for (int t = tid; t < p.n_mat * A; t += blockDim.x) {
+                const int m = t / A, a = t - m * A;
+                s_rden[t] = 1.f / (p.sig_t[m] + p.cdd[(part * A + a) * 4 + 3]);
+            }
+            cur_oct = o * 8 + part;
         }
 
         if (service) {
             // ------- service warp: publishes this item's progress, follows the upwind items' progress -------
             // It never joins the per-step barrier, so the latency of its global loads, fences and stores
             // stays off the other warps' critical path; the two sides talk through s_done / s_allowed.
-            const int *up_y = p.done + (g.has_y ? g.id - 1 : g.id), *up_z = p.done + (g.has_z ? g.id - p.ntj : g.id);
+            const int *up_y = p.done + (g.has_y ? g.id - p.a_split : g.id), *up_z = p.done + (g.has_z ? g.id - p.ntj * p.a_split : g.id);
             int *my_flag = p.done + g.id;
             int avail_y = g.has_y ? 0 : BIG, avail_z = g.has_z ? 0 : BIG;
             if (lane == 0) {
@@ -303,20 +316,6 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
             continue;
         }
 
-        if (tick) {
-            // ------- tick warp: counts the per-step barriers for the service warp -------
-            // It has no global memory traffic of its own, so its CTA-scope release costs nothing, while the
-            // same release issued by an aux or compute thread would wait for that warp's outstanding
-            // red.global / st.global round trips to L2 on every step.
-            __syncthreads();                          // S2
-            bar_compute(NB);                          // S3
-            for (int t = 0; t < T; ++t) {
-                bar_compute(NB);                      // B_t: every face store of step t precedes it
-                if (lane == 0) st_release_cta(&s_done, t + 1);
-            }
-            continue;
-        }
-
         // geometry of this lane's (j,k) column: its cell at step t is cbase + istep * t, for t - t_lo in [0, nx)
         const int jp = g.tj * DOS_TJ + jj, kp = g.tk * DOS_TK + kk;
         const bool valid = jp < ny && kp < nz;
@@ -326,39 +325,77 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
         const long long cbase = ((long long)k * ny + j) * nx + ((o & 1) ? nx - 1 : 0) - (long long)istep * skew;
         const int t_lo = valid ? skew : BIG;
 
-        if (aux) {
-            // ---------------- aux warps: staging, material ids, D2M of the previous step ----------------
-            const int xw = warp - NW, xt = tid - NW * 32, NXT = NX * 32;
-            const int n_ops = 32 * MV + 3 * A;
-            const LoadOp op0 = make_op<MP>(xt, p, g, s_q, s_fin);
-            const LoadOp op1 = make_op<MP>(xt + NXT < n_ops ? xt + NXT : xt, p, g, s_q, s_fin);
-            const bool op0_on = xt < n_ops, op1_on = xt + NXT < n_ops, more_ops = n_ops > 2 * NXT;
+        if (tick) {
+            // ------- feeder ("tick") warp: tile-inflow faces, material ids, step counter -------
+            // Copies the faces the upwind tiles have published (waiting for the service warp's word when they
+            // are not there yet), stages the material ids three steps ahead, and after every barrier tells the
+            // service warp how many steps are complete. Its CTA-scope release is cheap because its own global
+            // traffic is light; the same release from an aux or compute thread would wait for that warp's
+            // outstanding red.global / st.global round trips to L2 on every step.
+            const int n_fops = 3 * A;
+            const LoadOp op0 = make_op<MP>(32 * MV + (lane < n_fops ? lane : 0), p, g, s_q, s_fin);
+            const bool op0_on = lane < n_fops, more_ops = n_fops > 32;
             const uint8_t *mat_p = p.mat + cbase + 3 * istep;            // material of step t + 3
-            float *phi_p = p.phi + (cbase - istep) * MP;                 // moments of the cell of step t - 1
-            const int phi_inc = istep * MP;
-            const unsigned psi_r = smem_addr(s_psi + lane), d2m_a = smem_addr(s_d2m);
             const unsigned mat_w = smem_addr(s_mat + lane);
-            const int psi_slot = A * 32 * 4;
             auto mat_of = [&](int s, const uint8_t *q) -> int {
                 return ((unsigned)(s - t_lo) < (unsigned)nx) ? (int)__ldg(q) : 0;
             };
-            __syncthreads();                          // S2: octant tables, s_done, s_allowed in place
+            __syncthreads();                          // S2: s_done, s_allowed in place
             int allowed_c = -1;
-            auto gate = [&](int s) {                  // wait until the upwind tiles have published step s
-                while (allowed_c < s) {
-                    allowed_c = ld_acquire_cta(&s_allowed);
-                    if (allowed_c < s) __nanosleep(64);
-                }
-            };
             auto issue_one = [&](const LoadOp &d, int tau) {
-                const int s = tau + d.dist;
+                const int s = tau + DF;
                 if (s >= d.lo && s <= d.hi) {
-                    if (d.dist == DF) gate(s);
+                    while (allowed_c < s) {           // wait until the upwind tiles have published step s
+                        allowed_c = ld_acquire_cta(&s_allowed);
+                        if (allowed_c < s) __nanosleep(64);
+                    }
                     cp_async16(d.dst0 + (s & d.mask) * d.dslot, d.src0 + (long long)s * d.sstep);
                 }
             };
-            // round tau fetches the moments of step tau + DQ and the tile-inflow faces of step tau + DF
-            auto issue_round = [&](int tau) {
+            auto issue_round = [&](int tau) {         // round tau fetches the tile-inflow faces of step tau + DF
+                if (op0_on) issue_one(op0, tau);
+                if (more_ops)
+                    for (int f = lane + 32; f < n_fops; f += 32) issue_one(make_op<MP>(32 * MV + f, p, g, s_q, s_fin), tau);
+                cp_async_commit();
+            };
+            for (int tau = -DF; tau < 0; ++tau) issue_round(tau);
+            sts_s32(mat_w, mat_of(0, mat_p - 3 * istep));
+            sts_s32(mat_w + 128, mat_of(1, mat_p - 2 * istep));
+            int reg_m = mat_of(2, mat_p - istep);
+            cp_async_wait<DF - 1>();
+            bar_compute(NB);                          // S3: step 0's staged data visible to every warp
+#pragma unroll 1
+            for (int t = 0; t < T; ++t) {
+                trace_mark(trace, t, warp, 0);
+                issue_round(t);
+                sts_s32(mat_w + ((t + 2) & 3) * 128, reg_m);
+                reg_m = mat_of(t + 3, mat_p);
+                mat_p += istep;
+                cp_async_wait<DF - 1>();              // step t + 1's faces complete (this thread's copies)
+                trace_mark(trace, t, warp, 3);
+                bar_compute(NB);                      // B_t: ... visible to all; every face store of step t precedes it
+                if (lane == 0) st_release_cta(&s_done, t + 1);
+            }
+            continue;
+        }
+
+        if (aux) {
+            // ---------------- aux warps: staging, material ids, D2M of the previous step ----------------
+            const int xw = warp - NW, xt = tid - NW * 32, NXT = NX * 32;
+            const int n_ops = 32 * MV;                                   // Q copies; the feeder warp does the faces
+            const LoadOp op0 = make_op<MP>(xt < n_ops ? xt : 0, p, g, s_q, s_fin);
+            const LoadOp op1 = make_op<MP>(xt + NXT < n_ops ? xt + NXT : 0, p, g, s_q, s_fin);
+            const bool op0_on = xt < n_ops, op1_on = xt + NXT < n_ops, more_ops = n_ops > 2 * NXT;
+            float *phi_p = p.phi + (cbase - istep) * MP;                 // moments of the cell of step t - 1
+            const int phi_inc = istep * MP;
+            const unsigned psi_r = smem_addr(s_psi + lane), d2m_a = smem_addr(s_d2m);
+            const int psi_slot = A * 32 * 4;
+            __syncthreads();                          // S2: octant tables in place
+            auto issue_one = [&](const LoadOp &d, int tau) {
+                const int s = tau + DQ;
+                if (s >= d.lo && s <= d.hi) cp_async16(d.dst0 + (s & d.mask) * d.dslot, d.src0 + (long long)s * d.sstep);
+            };
+            auto issue_round = [&](int tau) {         // round tau fetches the source moments of step tau + DQ
                 if (op0_on) issue_one(op0, tau);
                 if (op1_on) issue_one(op1, tau);
                 if (more_ops)
@@ -366,23 +403,14 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
                 cp_async_commit();
             };
             for (int tau = -DQ; tau < 0; ++tau) issue_round(tau);
-            int reg_m = 0;
-            if (xw == 0) {
-                sts_s32(mat_w, mat_of(0, mat_p - 3 * istep));
-                sts_s32(mat_w + 128, mat_of(1, mat_p - 2 * istep));
-                reg_m = mat_of(2, mat_p - istep);
-            }
             cp_async_wait<DF - 1>();
             bar_compute(NB);                          // S3: step 0's staged data visible to every warp
 
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
+                trace_mark(trace, t, warp, 0);
                 issue_round(t);
-                if (xw == 0) {
-                    sts_s32(mat_w + ((t + 2) & 3) * 128, reg_m);
-                    reg_m = mat_of(t + 3, mat_p);
-                    mat_p += istep;
-                }
+                trace_mark(trace, t, warp, 1);
                 // D2M of step t - 1: sum over all angles of the octant, one red per (cell, 4 moments)
                 if (t > 0 && (unsigned)(t - 1 - t_lo) < (unsigned)nx) {
                     const unsigned ps = psi_r + ((t - 1) & 1) * psi_slot;
@@ -402,7 +430,9 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
                     }
                 }
                 phi_p += phi_inc;
+                trace_mark(trace, t, warp, 2);
                 cp_async_wait<DF - 1>();              // step t + 1's staged data complete (this thread's copies)
+                trace_mark(trace, t, warp, 3);
                 bar_compute(NB);                      // B_t: ... and visible to all
             }
             if ((unsigned)(T - 1 - t_lo) < (unsigned)nx) {
@@ -463,6 +493,7 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
 #pragma unroll 1
         for (int t = 0; t < T; ++t) {
             // moment-to-discrete for this lane's cell, AG angles; four partial sums keep the FMA chains short
+            trace_mark(trace, t, warp, 0);
             const bool act = (unsigned)(t - t_lo) < (unsigned)nx;
             const int m0 = lds_s32(mat_r + (t & 3) * 128);
             float q[AG];
@@ -487,6 +518,7 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
                 for (int r = 0; r < AG; ++r) q[r] = (part[r][0] + part[r][1]) + (part[r][2] + part[r][3]);
             }
 
+            trace_mark(trace, t, warp, 1);
             // inflow, diamond difference, outflow
             const unsigned fslot = (t & (RF - 1)) * fin_slot;
             const unsigned pso = psi_w + (t & 1) * psi_slot;
@@ -516,6 +548,8 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
                 sts_f32(pso + r * 128, pc);
             }
             fy_st += fy_inc; fz_st += fz_inc;
+            trace_mark(trace, t, warp, 2);
+            trace_mark(trace, t, warp, 3);
             bar_compute(NB);                          // B_t
         }
     }

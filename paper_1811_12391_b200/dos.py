@@ -22,6 +22,7 @@ STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_
 
 EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_solve",
            "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option", "dos_profile", "dos_profile_reset",
+           "dos_sweep_trace_host",
            "dos_destroy", "dos_last_error"]
 
 
@@ -75,6 +76,8 @@ _lib.dos_profile.restype = C.c_int
 _lib.dos_profile.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dos_profile_reset.restype = C.c_int
 _lib.dos_profile_reset.argtypes = [C.c_void_p]
+_lib.dos_sweep_trace_host.restype = C.c_int
+_lib.dos_sweep_trace_host.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
 _lib.dos_destroy.restype = None
 _lib.dos_destroy.argtypes = [C.c_void_p]
 _lib.dos_last_error.restype = C.c_char_p
@@ -208,6 +211,13 @@ class Context:
         self._check(_lib.dos_profile(self.handle, C.byref(p)))
         return {"sweep_ms": p.sweep_ms, "sweep_launches": p.sweep_launches, "raytrace_ms": p.raytrace_ms,
                 "raytrace_launches": p.raytrace_launches, "kernel_launches": p.kernel_launches}
+
+    def dos_sweep_trace_host(self):
+        """[steps][32 warps][4] int64 SM clocks of the traced sweep item (option sweep_trace_item)."""
+        steps = self.mesh["nx"] + 10
+        buf = np.zeros((steps, 32, 4), dtype=np.int64)
+        self._check(_lib.dos_sweep_trace_host(self.handle, buf.ctypes.data, buf.size))
+        return buf
 
     def dos_profile_reset(self):
         self._check(_lib.dos_profile_reset(self.handle))
