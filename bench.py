@@ -12,8 +12,10 @@ cell-angle-group updates/s over the whole step; `ms_per_step` is the cone-beam d
              between steps, max over ranks
   e2e        the same step through the C ABI with HOST buffers: material grid copied in from pinned
              memory (dos_set_material_host), dose map copied out (dos_dose_host), wall clock
-  roofline   the sweep kernel: algorithmic bytes per launch / its mean CUDA-event duration inside the
-             timed region, against MEASURED_PEAKS.json's HBM copy bandwidth
+  roofline   the sweep kernel: algorithmic flop per launch / its mean CUDA-event duration inside the
+             timed region, against the FP32 pipe peak (the sweep's arithmetic intensity is 4-13x the
+             ridge point); the same for algorithmic bytes against MEASURED_PEAKS.json's HBM copy
+             bandwidth under roofline.hbm
   cpu_baseline  the fp64 oracle, as it stands, on this box's host cores, on a bounded sample
 
 --impl reference times the oracle itself (there is no reference implementation: the paper's program is
@@ -279,10 +281,18 @@ def run_ours(args):
         flop = (4 * M + 12) * nv * n_ang
         rt_ms = prof["raytrace_ms"] / max(prof["raytrace_launches"], 1)
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "traffic.csv")     # ncu dram bytes per launch, copied from profiles/*.md
         if os.path.exists(tpath):
             with open(tpath) as f:
-                traffic = json.load(f).get(args.config, {}).get("sweep_dram_bytes_per_launch")
+                for row in f.read().splitlines()[1:]:
+                    c = row.split(",")
+                    if len(c) >= 3 and c[0] == args.config and c[1] == "sweep_kernel":
+                        traffic = int(c[2])
+        # FP32 pipe peak: SMs x 128 FP32 lanes x 2 flop x SM clock
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+        alu_peak = sms * 128 * 2 * mhz * 1e6 / 1e12
+        tflops = flop / (sweep_ms * 1e-3) / 1e12 if sweep_ms > 0 else 0.0
         line = {
             "metric": METRIC, "value": world * updates_per_step * args.steps / (total_ms * 1e-3), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
@@ -295,11 +305,14 @@ def run_ours(args):
                     "ms_per_step": e2e_total / args.steps * 1e3, "h2d_bytes_per_step": int(nv), "d2h_bytes_per_step": int(4 * nv)},
             "gpu_launches": int(prof["kernel_launches"]),
             "clocks": clocks,
-            "roofline": {"kernel": "sweep_kernel", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": sweep_bytes, "launch_ms": sweep_ms,
+            "roofline": {"kernel": "sweep_kernel", "bound": "alu", "achieved": tflops, "peak": alu_peak, "unit": "TFLOP/s",
+                         "frac": tflops / alu_peak, "traffic": traffic,
+                         "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 flop x {mhz:.0f} MHz (DESIGN.md section 7)",
+                         "algorithmic_flop_per_launch": flop,
+                         "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                                 "peak_source": peak_src, "algorithmic_bytes_per_launch": sweep_bytes},
+                         "launch_ms": sweep_ms,
                          "launches": int(prof["sweep_launches"]), "share_of_step": prof["sweep_ms"] / total_ms if total_ms else None,
-                         "fp32_tflops": flop / (sweep_ms * 1e-3) / 1e12 if sweep_ms > 0 else 0.0,
                          "updates_per_s_in_kernel": nv * n_ang / (sweep_ms * 1e-3) if sweep_ms > 0 else 0.0},
             "raytrace": {"launch_ms": rt_ms, "launches": int(prof["raytrace_launches"]),
                          "achieved_gbs": (nv * (1 + 4 * p["n_group"])) / (rt_ms * 1e-3) / 1e9 if rt_ms > 0 else 0.0,
