@@ -25,6 +25,8 @@ struct dos_ctx {
     int n_aux;                                         // aux warps of the sweep CTA
     int asplit, ag_pref, aux_pref;                     // angle split of an octant over CTAs; option overrides (0 = default)
     int trace_item;                                    // sweep work item whose timeline is recorded, or -1
+    int contraction_pref;                              // 0 auto, 1 FFMA (dos_sweep_ffma.cu), 2 tensor cores (dos_sweep.cu)
+    bool mma;                                          // the choice in force
     int impl;                                          // 0: dos_sweep.cu, 1: dos_sweep_v1.cu
     int ag1, n_grp1, chunk1, grid1;                    // the same for the first version
     size_t nv;
@@ -145,7 +147,7 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
     if (P_L > DOS_MAX_L) return fail(nullptr, DOS_ERR_UNSUPPORTED, "P_L > 5");
     if (q->n_ang < 8 || q->n_ang % 8 || !q->mu || !q->eta || !q->xi || !q->w)
         return fail(nullptr, DOS_ERR_INVALID_ARG, "n_ang must be a positive multiple of 8");
-    if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_v1_angles_per_warp(q->n_ang / 8, P_L) == 0)
+    if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_ffma_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_v1_angles_per_warp(q->n_ang / 8, P_L) == 0)
         return fail(nullptr, DOS_ERR_UNSUPPORTED, "angles per octant cannot be split over <= 12 warps of <= 4 angles");
     return DOS_OK;
 }
@@ -157,13 +159,17 @@ static cudaError_t configure_sweep(dos_ctx *c)
     int as = c->asplit;
     if (as < 1 || c->per_oct % as) as = 1;
     const int ap = c->per_oct / as;
-    const int ag = dos_sweep_angles_per_warp(ap, c->L, c->ag_pref);
-    if (ag == 0) return cudaErrorInvalidValue;
-    const int nx = dos_sweep_aux_warps(ap, c->L, ag, c->aux_pref);
+    // contractions on the tensor cores from P4 up (28 / 36 moments per cell), FFMA below (measured)
+    const bool mma = c->contraction_pref ? c->contraction_pref == 2 : dos_mpad(c->L) >= 28;
+    const int ag = mma ? dos_sweep_angles_per_warp(ap, c->L, c->ag_pref) : dos_sweep_ffma_angles_per_warp(ap, c->L, c->ag_pref);
+    if (ag == 0 || (c->ag_pref > 0 && ag != c->ag_pref)) return cudaErrorInvalidValue;
+    const int nx = mma ? dos_sweep_aux_warps(ap, c->L, ag, c->aux_pref) : dos_sweep_ffma_aux_warps(ap, c->L, ag, c->aux_pref);
+    if (ap / ag + nx + 2 > (mma ? 20 : 24)) return cudaErrorInvalidValue;
     int grid = 0;
-    cudaError_t e = dos_sweep_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, &grid);
+    cudaError_t e = mma ? dos_sweep_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, &grid)
+                        : dos_sweep_ffma_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, &grid);
     if (e != cudaSuccess) return e;
-    c->asplit = as; c->ag = ag; c->n_grp = ap / ag; c->n_aux = nx; c->grid = grid;
+    c->asplit = as; c->ag = ag; c->n_grp = ap / ag; c->n_aux = nx; c->grid = grid; c->mma = mma;
     return cudaSuccess;
 }
 
@@ -232,6 +238,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->n_items = 8 * c->ntj * c->ntk;
     c->impl = 0;
     c->trace_item = -1;
+    c->contraction_pref = 0;
     c->ag_pref = c->aux_pref = 0;
     c->asplit = default_asplit(per, c->n_items);
     c->chunk = 4;
@@ -465,7 +472,8 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
                                                  done, n_flags, queue, c->stream));
             prof_begin(c, 0);
             if (c->impl == 1) CUDA_TRY(c, dos_launch_sweep_v1(a1, c->L, c->ag1, c->grid1, c->stream));
-            else CUDA_TRY(c, dos_launch_sweep(a, c->L, c->ag, c->grid, c->stream));
+            else if (c->mma) CUDA_TRY(c, dos_launch_sweep(a, c->L, c->ag, c->grid, c->stream));
+            else CUDA_TRY(c, dos_launch_sweep_ffma(a, c->L, c->ag, c->grid, c->stream));
             prof_end(c);
             c->launches += 2;
         }
@@ -543,9 +551,7 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
         } else {
             c->aux_pref = (int)value;
         }
-        const bool bad_ag = c->ag_pref > 0 && dos_sweep_angles_per_warp(c->per_oct / c->asplit, c->L, c->ag_pref) != c->ag_pref;
-        cudaError_t e = bad_ag ? cudaErrorInvalidValue : configure_sweep(c);
-        if (e == cudaSuccess && c->n_grp + c->n_aux + 2 > 24) e = cudaErrorInvalidValue;
+        cudaError_t e = configure_sweep(c);
         if (e != cudaSuccess) {
             c->ag_pref = old_ag; c->aux_pref = old_aux; c->asplit = old_as;
             configure_sweep(c);
@@ -553,8 +559,22 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
         }
     } else if (!strcmp(name, "sweep_trace_item")) {
         if (value < -1 || value >= c->n_items * c->asplit) return fail(c, DOS_ERR_INVALID_ARG, "sweep_trace_item out of range");
+        if (value >= 0 && !dos_sweep_trace_compiled())
+            return fail(c, DOS_ERR_UNSUPPORTED, "sweep_trace_item: libdos was built without -DDOS_SWEEP_TRACE=1");
         c->trace_item = (int)value;
         CUDA_TRY(c, cudaMemsetAsync(c->ws + c->lay.trace, 0, sizeof(long long) * (size_t)(c->mesh.nx + DOS_SKEW) * 128, c->stream));
+    } else if (!strcmp(name, "sweep_contraction")) {
+        if (value < 0 || value > 2) return fail(c, DOS_ERR_INVALID_ARG, "sweep_contraction must be 0 (auto), 1 (FFMA) or 2 (tensor cores)");
+        const int old = c->contraction_pref;
+        c->contraction_pref = (int)value;
+        if (configure_sweep(c) != cudaSuccess) {
+            c->contraction_pref = old;
+            configure_sweep(c);
+            return fail(c, DOS_ERR_INVALID_ARG, "sweep_contraction: not admissible with the current sweep shape options");
+        }
+    } else if (!strcmp(name, "sweep_two_per_sm")) {
+        dos_sweep_set_two_per_sm(value != 0);
+        CUDA_TRY(c, configure_sweep(c));
     } else if (!strcmp(name, "profile")) {
         c->profile = value != 0;
     } else if (!strcmp(name, "sweep_grid")) {
