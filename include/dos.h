@@ -143,8 +143,9 @@ dos_status dos_check(dos_ctx *ctx);
  *                   CTAs an octant's angles are spread over (0 = library default)
  *   "sweep_contraction"  where the sweep's moment-to-discrete / discrete-to-moment contractions run: 0 (default)
  *                   tensor cores (3xTF32 mma.sync) from P4 up and FFMA below, 1 FFMA, 2 tensor cores
- *   "sweep_two_per_sm"  1: small problems (<= 16 moments, more work items than SMs) use the sweep variant
- *                   capped at 64 registers so that two CTAs share an SM; 0 (default: measured slower on config 2): never. Process-wide.
+ *   "sweep_two_per_sm"  bit 0: tensor-core sweep, bit 1: FFMA sweep (default 2). Where set, problems of <= 16
+ *                   moments per cell use a sweep variant capped at 64 registers so that two CTAs share an SM (FFMA
+ *                   sweep: only with >= 4 work items per SM). Process-wide.
  *   "sweep_impl"    0: dos_sweep.cu (default), 1: the first version kept for A/B measurements
  *   "sweep_trace_item"  see dos_sweep_trace_host
  *   "profile"       1: bracket every sweep and ray-trace launch with CUDA events (see dos_profile)  */

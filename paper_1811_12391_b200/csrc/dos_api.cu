@@ -573,7 +573,8 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
             return fail(c, DOS_ERR_INVALID_ARG, "sweep_contraction: not admissible with the current sweep shape options");
         }
     } else if (!strcmp(name, "sweep_two_per_sm")) {
-        dos_sweep_set_two_per_sm(value != 0);
+        dos_sweep_set_two_per_sm(value & 1);       // bit 0: tensor-core sweep, bit 1: FFMA sweep
+        dos_sweep_ffma_set_two_per_sm((value & 4) ? 2 : ((value & 2) ? 1 : 0));   // bit 2: also for few items per SM
         CUDA_TRY(c, configure_sweep(c));
     } else if (!strcmp(name, "profile")) {
         c->profile = value != 0;

@@ -88,5 +88,6 @@ cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ang_per_warp, 
 int dos_sweep_ffma_angles_per_warp(int per_oct, int L, int prefer);
 cudaError_t dos_sweep_ffma_grid(int L, int ang_per_warp, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out);
 int dos_sweep_ffma_aux_warps(int per_oct, int L, int ang_per_warp, int prefer);
+void dos_sweep_ffma_set_two_per_sm(int on);
 void dos_sweep_set_two_per_sm(int on);   // allow the 64-register, 2-CTAs-per-SM variant (process-wide)
 int dos_sweep_trace_compiled();   // 1 if dos_sweep.cu was built with -DDOS_SWEEP_TRACE=1

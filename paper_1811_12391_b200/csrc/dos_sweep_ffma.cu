@@ -220,8 +220,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
 //                                 service warp
 //   service warp   NW + NX + 1    global hand-off flags (never joins the per-step barrier)
 // TMAX = CTA size bound for the register budget.
-template <int MP, int AG, int TMAX>
-__global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
+template <int MP, int AG, int TMAX, int MINB>
+__global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
 {
     constexpr int MV = MP / 4, MPS = mps_of(MP);
     extern __shared__ float4 smem4[];
@@ -574,28 +574,44 @@ __global__ void __launch_bounds__(TMAX) sweep_kernel(const Sweep2Args p)
 // ------------------------------------------------------------------------------------------------
 typedef void (*sweep_fn)(const Sweep2Args);
 
+// variant 0: up to 16 warps, 1 CTA per SM; 1: up to 24 warps; 2: up to 16 warps capped at 64 registers so that two
+// CTAs share an SM (MP <= 16 only) -- on meshes with many more work items than SMs the second CTA fills the other's
+// barrier and latency stalls (config 4: measured in DESIGN.md section 6)
+template <int MP, int AG>
+static sweep_fn pick_var(int var)
+{
+    if (var == 1) return sweep_kernel<MP, AG, 768, 1>;
+    if (var == 2) return MP <= 16 ? sweep_kernel<(MP <= 16 ? MP : 4), AG, 512, 2> : nullptr;
+    return sweep_kernel<MP, AG, 512, 1>;
+}
+
 template <int MP>
-static sweep_fn pick_ag(int ag, bool big)
+static sweep_fn pick_ag(int ag, int var)
 {
     switch (ag) {
-        case 1: return big ? sweep_kernel<MP, 1, 768> : sweep_kernel<MP, 1, 512>;
-        case 2: return big ? sweep_kernel<MP, 2, 768> : sweep_kernel<MP, 2, 512>;
-        case 3: return big ? sweep_kernel<MP, 3, 768> : sweep_kernel<MP, 3, 512>;
-        case 4: return big ? sweep_kernel<MP, 4, 768> : sweep_kernel<MP, 4, 512>;
+        case 1: return pick_var<MP, 1>(var);
+        case 2: return pick_var<MP, 2>(var);
+        case 3: return pick_var<MP, 3>(var);
+        case 4: return pick_var<MP, 4>(var);
     }
     return nullptr;
 }
 
-// CTAs of more than 16 warps (compute + aux + service) need the 768-thread variant
-static sweep_fn pick(int L, int ag, int per_oct, int n_aux)
+static int g_two_per_sm = 1;     // 1: variant 2 from 4 work items per SM, 2: whenever there are more items than SMs, 0: never
+void dos_sweep_ffma_set_two_per_sm(int on) { g_two_per_sm = on; }
+
+static sweep_fn pick(int L, int ag, int per_oct, int n_aux, int n_items)
 {
-    const bool big = per_oct / ag + n_aux + 2 > 16;
-    switch (dos_mpad(L)) {
-        case 4: return pick_ag<4>(ag, big);
-        case 12: return pick_ag<12>(ag, big);
-        case 16: return pick_ag<16>(ag, big);
-        case 28: return pick_ag<28>(ag, big);
-        case 36: return pick_ag<36>(ag, big);
+    const int warps = per_oct / ag + n_aux + 2, MP = dos_mpad(L);
+    int sms = 148, dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int var = warps > 16 ? 1 : ((g_two_per_sm && MP <= 16 && (g_two_per_sm == 2 ? n_items > sms : n_items >= 4 * sms)) ? 2 : 0);
+    switch (MP) {
+        case 4: return pick_ag<4>(ag, var);
+        case 12: return pick_ag<12>(ag, var);
+        case 16: return pick_ag<16>(ag, var);
+        case 28: return pick_ag<28>(ag, var);
+        case 36: return pick_ag<36>(ag, var);
     }
     return nullptr;
 }
@@ -636,7 +652,7 @@ int dos_sweep_ffma_angles_per_warp(int per_oct, int L, int prefer)
 
 cudaError_t dos_sweep_ffma_grid(int L, int ag, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out)
 {
-    sweep_fn f = pick(L, ag, per_oct, n_aux);
+    sweep_fn f = pick(L, ag, per_oct, n_aux, n_items);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, per_oct, n_mat);
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -656,7 +672,7 @@ cudaError_t dos_sweep_ffma_grid(int L, int ag, int n_aux, int per_oct, int n_mat
 
 cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ag, int grid, cudaStream_t s)
 {
-    sweep_fn f = pick(L, ag, a.per_oct, a.n_aux);
+    sweep_fn f = pick(L, ag, a.per_oct, a.n_aux, a.n_items);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, a.per_oct, a.n_mat);
     f<<<grid, (a.n_warps + a.n_aux + 2) * 32, smem, s>>>(a);
