@@ -47,7 +47,12 @@ cudaError_t dos_sweep_v1_grid(int L, int ang_per_warp, int per_oct, int n_mat, i
 #define DOS_FACE_PAD 8      // diagonal index d = x + (lane offset) runs over [0, nx + DOS_FACE_PAD)
 #define DOS_PREFETCH_Q 6    // steps between issuing the cp.async of a step's source moments and using them
 #define DOS_RING_Q 8
-#define DOS_PREFETCH_F 3    // the same for tile-inflow faces
+#ifndef DOS_PREFETCH_F
+#define DOS_PREFETCH_F 2    // the same for tile-inflow faces (each step of it is a step of hand-off lag per tile hop)
+#endif
+#ifndef DOS_POLL_NS
+#define DOS_POLL_NS 64      // pause between polls of a hand-off flag / of the shared progress words
+#endif
 #define DOS_RING_F 4
 
 // Arguments of one launch (all 8 octants, one energy group, one source iteration).

@@ -448,10 +448,10 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
                             avail_y = avail_z = BIG;
                             if (lane == 0) st_release_cta(&s_allowed, BIG);
                         }
-                        __nanosleep(64);
+                        __nanosleep(DOS_POLL_NS);
                     }
                 } else {
-                    __nanosleep(128);
+                    __nanosleep(2 * DOS_POLL_NS);
                 }
             }
             continue;
@@ -488,7 +488,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
                 if (s >= d.lo && s <= d.hi) {
                     while (allowed_c < s) {           // wait until the upwind tiles have published step s
                         allowed_c = ld_acquire_cta(&s_allowed);
-                        if (allowed_c < s) __nanosleep(64);
+                        if (allowed_c < s) __nanosleep(DOS_POLL_NS);
                     }
                     cp_async16(d.dst0 + (s & d.mask) * d.dslot, d.src0 + (long long)s * d.sstep);
                 }

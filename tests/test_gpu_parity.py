@@ -54,6 +54,43 @@ def test_small_problem_parity(dos, orc, name, ov):
     assert_problem_parity(out, ref, name)
 
 
+# Every sweep implementation on every kind of problem, whatever the library's default choice is: FFMA contractions
+# (dos_sweep_ffma.cu), tensor-core contractions (dos_sweep.cu), the 64-register two-CTAs-per-SM variants, 8 aux warps.
+SWEEP_VARIANTS = [
+    ("ffma", {"sweep_contraction": 1, "sweep_two_per_sm": 0}),
+    ("ffma-2cta", {"sweep_contraction": 1, "sweep_two_per_sm": 6}),
+    ("mma", {"sweep_contraction": 2, "sweep_two_per_sm": 0}),
+    ("mma-2cta", {"sweep_contraction": 2, "sweep_two_per_sm": 1}),
+    ("mma-8aux", {"sweep_contraction": 2, "sweep_aux_warps": 8}),
+    ("v1", {"sweep_impl": 1}),
+]
+VARIANT_CASES = [
+    ("config2", dict(nx=37, ny=21, nz=10, voxel=1.0, n_group=4, n_iter=4)),                        # S8/P3, ragged tiles
+    ("config3", dict(nx=26, ny=20, nz=9, voxel=1.5, n_group=3, n_iter=3)),                         # S16/P5
+    ("config2", dict(nx=33, ny=9, nz=5, voxel=1.1, n_group=3, n_iter=3, sn=6, pl=2)),              # S6/P2 (M padded 9->12)
+]
+
+
+@pytest.mark.parametrize("case", range(len(VARIANT_CASES)))
+def test_every_sweep_variant_parity(dos, orc, case):
+    name, ov = VARIANT_CASES[case]
+    p = _make(name, **ov)
+    ref = orc.run_problem(p)
+    try:
+        for label, opts in SWEEP_VARIANTS:
+            ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+            for k, v in opts.items():
+                ctx.dos_set_option(k, v)
+            out = dos.run_problem(p, ctx=ctx)
+            ctx.close()
+            assert_problem_parity(out, ref, f"{name} [{label}]")
+    finally:
+        # sweep_two_per_sm is process-wide: back to the library default
+        ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+        ctx.dos_set_option("sweep_two_per_sm", 2)
+        ctx.close()
+
+
 def test_config2_full_parity(dos, orc):
     """BASELINE.json configs[1] at full size and full iteration count."""
     p = _make("config2")
