@@ -316,6 +316,7 @@ def run_ours(args):
                          "updates_per_s_in_kernel": nv * n_ang / (sweep_ms * 1e-3) if sweep_ms > 0 else 0.0},
             "raytrace": {"launch_ms": rt_ms, "launches": int(prof["raytrace_launches"]),
                          "achieved_gbs": (nv * (1 + 4 * p["n_group"])) / (rt_ms * 1e-3) / 1e9 if rt_ms > 0 else 0.0,
+                         "hbm_frac": (nv * (1 + 4 * p["n_group"])) / (rt_ms * 1e-3) / 1e9 / peak if rt_ms > 0 else 0.0,
                          "voxels_per_s": nv / (rt_ms * 1e-3) if rt_ms > 0 else 0.0},
         }
         if not args.no_cpu_baseline:
