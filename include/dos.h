@@ -82,7 +82,8 @@ typedef struct {
     int32_t isotropic;
 } dos_source;
 
-/* Bytes of device workspace dos_create needs for this problem (n_batch must be 1 in this build). */
+/* Bytes of device workspace dos_create needs for this problem. n_batch = 1: one source per solve; n_batch > 1:
+ * also the buffers of the summed-source mode (dos_uncollided_sum): [G][Nv][MP] + [G][Nv] floats more. */
 dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs, const dos_quadrature *quad,
                                int32_t P_L, int32_t n_batch, size_t *bytes_out);
 
@@ -111,6 +112,18 @@ dos_status dos_set_material_host(dos_ctx *ctx, const uint8_t *h_material_ids);
  *   d_phi_u_out     device [G][nz][ny][nx] or NULL: also copy the result there                      */
 dos_status dos_uncollided(dos_ctx *ctx, const dos_source *source, const float *spectrum,
                           float *d_phi_u_out);
+
+/* Summed-source mode (the cone beams of a CT scan form ONE source and
+ * the S_N equations are solved once). Like dos_uncollided, but the uncollided fluence of this source is ADDED to
+ * that of the sources given since the last call with first != 0: phi_u = sum_p phi_u,p, and the first-collision
+ * source of the following dos_solve is sum_p Y_lm(Omega_p) sum_{g'<=g} sigma_sl^{g'->g} phi_u,p^{g'} (each position
+ * with its own direction Omega_p from the source to the cell). first != 0 starts a new sum. dos_fluence and
+ * dos_dose then report the summed uncollided fluence plus the one collided solution. By linearity this equals the
+ * sum of the per-position solves wherever the negative-flux fixup does not fire; it is NOT config 4's
+ * sum of separate solves. d_phi_u_out (device [G][nz][ny][nx], may be NULL) receives this source's own phi_u.
+ * Needs a workspace sized by dos_workspace_bytes with n_batch > 1 (else DOS_ERR_STATE). */
+dos_status dos_uncollided_sum(dos_ctx *ctx, const dos_source *source, const float *spectrum, int32_t first,
+                              float *d_phi_u_out);
 
 /* Collided fluence (PAPER.md:39-45 eq. 2-3, :49): for g = 0..G-1, top-down (downscatter only):
  *   Q_fix = first-collision source moments Y_lm(Omega_r) sum_{g'<=g} sigma_sl^{g'->g} phi_u^{g'}

@@ -199,3 +199,38 @@ def run_problem(p, source_index=0, n_iter=None):
                      p["n_iter"] if n_iter is None else n_iter, source_pos=src["pos"], phi_u=pu, want_abs=True)
     tot, d = dose(p["mesh"], p["material"], p["kerma"], pu, pc)
     return {"phi_u": pu, "phi_c": pc[:, 0], "phi_total": tot, "dose": d, "phi_c_moments": pc, "phi_c_abs": pabs}
+
+
+def first_collision(mesh, material, sigma_s, L, source_pos, phi_u, q_out):
+    """ADDS the first-collision source moments of one source position (O2) into q_out
+    [G][M][nz*ny*nx] (float64): q_out[g][lm] += Y_lm(Omega_r) sum_{g'<=g} sigma_sl^{g'->g} phi_u^{g'}."""
+    sig_s = _d(sigma_s)
+    n_leg, G = sig_s.shape[1] - 1, sig_s.shape[2]
+    mat = np.ascontiguousarray(material, dtype=np.uint8)
+    pu = _d(phi_u).reshape(G, mat.size)
+    pos = _d(source_pos)
+    ms = _mesh(mesh)
+    assert q_out.dtype == np.float64 and q_out.flags.c_contiguous and q_out.shape == (G, n_moments(L), mat.size)
+    for g in range(G):
+        lib().orc_first_collision(C.byref(ms), _p(mat), C.c_int(G), C.c_int(n_leg), C.c_int(L), _p(sig_s), _p(pos), _p(pu),
+                                  C.c_int(g), C.c_void_p(q_out[g].ctypes.data))
+
+
+def run_problem_summed(p, source_indices=None, n_iter=None):
+    """the given source positions form ONE source. The uncollided fluence
+    and the first-collision source moments of the positions are summed (each position with its own direction to
+    the cell), then O3-O5 run once. Same keys as run_problem; phi_u is the summed uncollided fluence."""
+    idx = list(range(len(p["sources"]))) if source_indices is None else list(source_indices)
+    mat = np.ascontiguousarray(p["material"], dtype=np.uint8)
+    G, M = np.asarray(p["sigma_t"]).shape[1], n_moments(p["P_L"])
+    q_ext = np.zeros((G, M, mat.size))
+    pu_sum = np.zeros((G,) + mat.shape)
+    for s in idx:
+        src = p["sources"][s]
+        pu = uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+        pu_sum += pu
+        first_collision(p["mesh"], p["material"], p["sigma_s"], p["P_L"], src["pos"], pu, q_ext)
+    pc, pabs = solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"],
+                     p["n_iter"] if n_iter is None else n_iter, phi_u=None, q_ext=q_ext, want_abs=True)
+    tot, d = dose(p["mesh"], p["material"], p["kerma"], pu_sum, pc)
+    return {"phi_u": pu_sum, "phi_c": pc[:, 0], "phi_total": tot, "dose": d, "phi_c_moments": pc, "phi_c_abs": pabs}

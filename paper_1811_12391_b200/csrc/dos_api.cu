@@ -15,7 +15,7 @@
 
 struct Layout {
     size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
-        spectrum, errflag, trace, total;
+        spectrum, errflag, trace, um, phi_u_sum, total;
 };
 
 struct dos_ctx {
@@ -36,6 +36,7 @@ struct dos_ctx {
     Layout lay;
     std::vector<int> band_lo;    // [G]: lowest g' with a non-zero sigma_s^{g'->g}
     int state;                   // 0 created, 1 uncollided done, 2 solved
+    bool can_sum, summed;        // workspace holds the summed-source buffers; the current uncollided state is a sum
     dos_source src;
     bool have_dose_acc;
     bool profile, prof_open;
@@ -95,7 +96,7 @@ static void host_ylm(double mu, double eta, double xi, int L, double *y)
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
-static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L, int n_ang)
+static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L, int n_ang, bool summed)
 {
     Layout l;
     const size_t nv = (size_t)m->nx * m->ny * m->nz;
@@ -129,6 +130,9 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.spectrum = take(sizeof(double) * G);
     l.errflag = take(sizeof(int) * 4);
     l.trace = take(sizeof(long long) * (size_t)(m->nx + DOS_SKEW) * 32 * 4);
+    // summed-source mode (dos_uncollided_sum): uncollided moments of all positions and their scalar sum
+    l.um = summed ? take(sizeof(float) * G * nv * MP) : 0;
+    l.phi_u_sum = summed ? take(sizeof(float) * G * nv) : 0;
     l.total = off;
     return l;
 }
@@ -188,8 +192,8 @@ extern "C" dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs
     if (!bytes_out) return fail(nullptr, DOS_ERR_INVALID_ARG, "bytes_out is null");
     dos_status s = check_inputs(mesh, xs, quad, P_L);
     if (s != DOS_OK) return s;
-    if (n_batch != 1) return fail(nullptr, DOS_ERR_UNSUPPORTED, "n_batch must be 1");
-    *bytes_out = make_layout(mesh, xs->n_mat, xs->n_group, xs->n_leg, P_L, quad->n_ang).total;
+    if (n_batch < 1) return fail(nullptr, DOS_ERR_INVALID_ARG, "n_batch must be >= 1");
+    *bytes_out = make_layout(mesh, xs->n_mat, xs->n_group, xs->n_leg, P_L, quad->n_ang, n_batch > 1).total;
     return DOS_OK;
 }
 
@@ -226,7 +230,10 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
                 quad->eta[n] != ey || quad->xi[n] != ez || quad->w[n] != quad->w[t])
                 return fail(nullptr, DOS_ERR_INVALID_ARG, "quadrature is not octant-major / octant-symmetric");
         }
-    Layout lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang);
+    // a workspace sized with n_batch > 1 also holds the buffers of the summed-source mode
+    Layout lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang, true);
+    const bool can_sum = workspace_bytes >= lay.total;
+    if (!can_sum) lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang, false);
     if (workspace_bytes < lay.total) return fail(nullptr, DOS_ERR_SHAPE, "workspace too small");
 
     dos_ctx *c = new (std::nothrow) dos_ctx();
@@ -238,6 +245,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->n_items = 8 * c->ntj * c->ntk;
     c->impl = 0;
     c->trace_item = -1;
+    c->can_sum = can_sum; c->summed = false;
     c->contraction_pref = 0;
     c->ag_pref = c->aux_pref = 0;
     c->asplit = default_asplit(per, c->n_items);
@@ -384,9 +392,12 @@ extern "C" dos_status dos_set_material_host(dos_ctx *c, const uint8_t *h_materia
     return DOS_OK;
 }
 
-extern "C" dos_status dos_uncollided(dos_ctx *c, const dos_source *source, const float *spectrum, float *d_phi_u_out)
+// mode 0: single source; 1: first source of a sum; 2: further source of a sum
+static dos_status uncollided_impl(dos_ctx *c, const dos_source *source, const float *spectrum, float *d_phi_u_out, int mode)
 {
     if (!c || !source || !spectrum) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    if (mode && !c->can_sum) return fail(c, DOS_ERR_STATE, "the workspace was not sized for the summed-source mode (dos_workspace_bytes with n_batch > 1)");
+    if (mode == 2 && !(c->summed && c->state >= 1)) return fail(c, DOS_ERR_STATE, "dos_uncollided_sum(first = 0) without a first source");
     auto dot = [](const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; };
     if (!source->isotropic) {
         if (std::fabs(dot(source->axis, source->axis) - 1.0) > 1e-9 || std::fabs(dot(source->up, source->up) - 1.0) > 1e-9 ||
@@ -422,10 +433,27 @@ extern "C" dos_status dos_uncollided(dos_ctx *c, const dos_source *source, const
                                     phi_u, (int *)(c->ws + c->lay.errflag), c->stream));
     prof_end(c);
     c->launches += 1;
+    if (mode) {
+        CUDA_TRY(c, dos_launch_um_accumulate(mesh_dev(c->mesh), source_dev(*source), c->G, c->L, mode == 1, phi_u,
+                                             (float *)(c->ws + c->lay.um), (float *)(c->ws + c->lay.phi_u_sum), c->stream));
+        c->launches += 1;
+    }
+    c->summed = mode != 0;
     if (d_phi_u_out)
         CUDA_TRY(c, cudaMemcpyAsync(d_phi_u_out, phi_u, sizeof(float) * c->G * c->nv, cudaMemcpyDeviceToDevice, c->stream));
     c->state = 1;
     return DOS_OK;
+}
+
+extern "C" dos_status dos_uncollided(dos_ctx *c, const dos_source *source, const float *spectrum, float *d_phi_u_out)
+{
+    return uncollided_impl(c, source, spectrum, d_phi_u_out, 0);
+}
+
+extern "C" dos_status dos_uncollided_sum(dos_ctx *c, const dos_source *source, const float *spectrum, int32_t first,
+                                         float *d_phi_u_out)
+{
+    return uncollided_impl(c, source, spectrum, d_phi_u_out, first ? 1 : 2);
 }
 
 extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
@@ -463,6 +491,7 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
         CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
+                                            c->summed ? (const float *)(c->ws + c->lay.um) : nullptr,
                                             phi_all, qfix, c->stream));
         c->launches += 1;
         a.phi = a1.phi = phi;
@@ -502,7 +531,7 @@ extern "C" dos_status dos_fluence(dos_ctx *c, float *d_phi_collided, float *d_ph
 {
     if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
     if (c->state < 2) return fail(c, DOS_ERR_STATE, "dos_fluence before dos_solve");
-    CUDA_TRY(c, dos_launch_fluence(c->nv, c->G, c->MP, (const float *)(c->ws + c->lay.phi_u),
+    CUDA_TRY(c, dos_launch_fluence(c->nv, c->G, c->MP, (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u)),
                                    (const float *)(c->ws + c->lay.phi_all), d_phi_collided, d_phi_total, c->stream));
     c->launches += 1;
     return DOS_OK;
@@ -513,7 +542,7 @@ extern "C" dos_status dos_dose(dos_ctx *c, float *d_dose, int32_t accumulate)
     if (!c || !d_dose) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
     if (c->state < 2) return fail(c, DOS_ERR_STATE, "dos_dose before dos_solve");
     CUDA_TRY(c, dos_launch_dose(c->nv, c->d_mat, c->n_mat, c->G, c->MP, (const float *)(c->ws + c->lay.kerma),
-                                (const float *)(c->ws + c->lay.phi_u), (const float *)(c->ws + c->lay.phi_all), d_dose,
+                                (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u)), (const float *)(c->ws + c->lay.phi_all), d_dose,
                                 accumulate, c->stream));
     c->launches += 1;
     return DOS_OK;

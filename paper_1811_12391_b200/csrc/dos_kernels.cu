@@ -153,6 +153,7 @@ __global__ void __launch_bounds__(128) group_source_kernel(MeshDev m, SourceDev 
                                                            int G, int n_leg, int g, int g_lo,
                                                            const float *__restrict__ sig_s,
                                                            const float *__restrict__ phi_u,
+                                                           const float *__restrict__ um,
                                                            const float *__restrict__ phi_all, float *__restrict__ qfix)
 {
     constexpr int M = (L + 1) * (L + 1), MP = (M + 3) & ~3;
@@ -169,7 +170,7 @@ __global__ void __launch_bounds__(128) group_source_kernel(MeshDev m, SourceDev 
     bool any = false;
 #pragma unroll
     for (int l = 0; l <= L; ++l) sl[l] = 0.f;
-    for (int gp = 0; gp <= g; ++gp) {
+    for (int gp = 0; um == nullptr && gp <= g; ++gp) {
         const float pu = phi_u[(size_t)gp * nv + cell];
         if (pu != 0.f) {
             any = true;
@@ -189,9 +190,12 @@ __global__ void __launch_bounds__(128) group_source_kernel(MeshDev m, SourceDev 
 #pragma unroll
             for (int mm = -l; mm <= l; ++mm) acc[l * (l + 1) + mm] = y[l * (l + 1) + mm] * sl[l];
     }
-    // downscatter from the collided fluence of the groups above (banded)
-    for (int gp = g_lo; gp < g; ++gp) {
-        const float4 *pp = reinterpret_cast<const float4 *>(phi_all + ((size_t)gp * nv + cell) * MP);
+    // downscatter from the collided fluence of the groups above (banded); in summed-source mode
+    // also the first-collision source from the uncollided moments U^{g'}[lm] = sum_p Y_lm(Omega_p) phi_u,p^{g'} of
+    // all source positions, g' <= g
+    for (int pass = (um ? 0 : 1); pass < 2; ++pass)
+    for (int gp = g_lo; gp < g + (pass == 0 ? 1 : 0); ++gp) {
+        const float4 *pp = reinterpret_cast<const float4 *>((pass == 0 ? um : phi_all) + ((size_t)gp * nv + cell) * MP);
         float sg[L + 1];
 #pragma unroll
         for (int l = 0; l <= L; ++l) sg[l] = ss[((size_t)l * G + gp) * G + g];
@@ -278,18 +282,18 @@ __global__ void dose_kernel(size_t nv, const uint8_t *__restrict__ mat, int G, i
 }  // namespace
 
 cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int G, int n_leg, int L,
-                                    int g, int g_lo, const float *sig_s, const float *phi_u, const float *phi_all,
-                                    float *qfix, cudaStream_t st)
+                                    int g, int g_lo, const float *sig_s, const float *phi_u, const float *um,
+                                    const float *phi_all, float *qfix, cudaStream_t st)
 {
     const size_t nv = (size_t)m.nx * m.ny * m.nz;
     const unsigned grid = (unsigned)((nv + 127) / 128);
     switch (L) {
-        case 0: group_source_kernel<0><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, phi_all, qfix); break;
-        case 1: group_source_kernel<1><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, phi_all, qfix); break;
-        case 2: group_source_kernel<2><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, phi_all, qfix); break;
-        case 3: group_source_kernel<3><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, phi_all, qfix); break;
-        case 4: group_source_kernel<4><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, phi_all, qfix); break;
-        case 5: group_source_kernel<5><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, phi_all, qfix); break;
+        case 0: group_source_kernel<0><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 1: group_source_kernel<1><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 2: group_source_kernel<2><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 3: group_source_kernel<3><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 4: group_source_kernel<4><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 5: group_source_kernel<5><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -305,6 +309,74 @@ cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int G, int n
     const unsigned grid = (unsigned)((n + 255) / 256);
     source_update_kernel<<<grid, 256, 0, st>>>(nv, MV, M, mat, G, n_leg, g, sig_s, (const float4 *)qfix, (float4 *)phi,
                                                (float4 *)q, first, done, n_flags, queue);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Summed-source mode (the cone beams of a CT scan form ONE source and are swept
+// once). After the ray trace of position p: U^g[lm](c) (+)= Y_lm(Omega_p(c)) phi_u,p^g(c) and
+// phi_u_sum^g(c) (+)= phi_u,p^g(c). One thread per cell; `first` overwrites instead of adding.
+// ------------------------------------------------------------------------------------------------
+template <int L>
+__global__ void __launch_bounds__(128) um_accumulate_kernel(MeshDev m, SourceDev s, int G, int first,
+                                                            const float *__restrict__ phi_u_pos, float *__restrict__ um,
+                                                            float *__restrict__ phi_u_sum)
+{
+    constexpr int M = (L + 1) * (L + 1), MP = (M + 3) & ~3;
+    const size_t nv = (size_t)m.nx * m.ny * m.nz;
+    const size_t cell = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= nv) return;
+    bool any = false;
+    for (int g = 0; g < G; ++g) any |= phi_u_pos[(size_t)g * nv + cell] != 0.f;
+    if (!any && !first) return;
+    float y[MP];
+#pragma unroll
+    for (int t = 0; t < MP; ++t) y[t] = 0.f;
+    if (any) {
+        const int i = (int)(cell % m.nx), j = (int)((cell / m.nx) % m.ny), k = (int)(cell / ((size_t)m.nx * m.ny));
+        const double dx = m.x0 + (i + 0.5) * m.dx - s.pos[0], dy = m.y0 + (j + 0.5) * m.dy - s.pos[1],
+                     dz = m.z0 + (k + 0.5) * m.dz - s.pos[2];
+        const double rinv = rsqrt(dx * dx + dy * dy + dz * dz);
+        float yy[M];
+        dev_ylm<L>(dx * rinv, dy * rinv, dz * rinv, yy);
+#pragma unroll
+        for (int t = 0; t < M; ++t) y[t] = yy[t];
+    }
+    for (int g = 0; g < G; ++g) {
+        const float pu = phi_u_pos[(size_t)g * nv + cell];
+        float4 *up = reinterpret_cast<float4 *>(um + ((size_t)g * nv + cell) * MP);
+        float *ps = phi_u_sum + (size_t)g * nv + cell;
+        if (first) {
+            *ps = pu;
+#pragma unroll
+            for (int v = 0; v < MP / 4; ++v) up[v] = make_float4(y[4 * v] * pu, y[4 * v + 1] * pu, y[4 * v + 2] * pu, y[4 * v + 3] * pu);
+        } else if (pu != 0.f) {
+            *ps += pu;
+#pragma unroll
+            for (int v = 0; v < MP / 4; ++v) {
+                float4 u = up[v];
+                u.x = fmaf(y[4 * v], pu, u.x); u.y = fmaf(y[4 * v + 1], pu, u.y);
+                u.z = fmaf(y[4 * v + 2], pu, u.z); u.w = fmaf(y[4 * v + 3], pu, u.w);
+                up[v] = u;
+            }
+        }
+    }
+}
+
+cudaError_t dos_launch_um_accumulate(const MeshDev &m, const SourceDev &s, int G, int L, int first, const float *phi_u_pos,
+                                     float *um, float *phi_u_sum, cudaStream_t st)
+{
+    const size_t nv = (size_t)m.nx * m.ny * m.nz;
+    const unsigned grid = (unsigned)((nv + 127) / 128);
+    switch (L) {
+        case 0: um_accumulate_kernel<0><<<grid, 128, 0, st>>>(m, s, G, first, phi_u_pos, um, phi_u_sum); break;
+        case 1: um_accumulate_kernel<1><<<grid, 128, 0, st>>>(m, s, G, first, phi_u_pos, um, phi_u_sum); break;
+        case 2: um_accumulate_kernel<2><<<grid, 128, 0, st>>>(m, s, G, first, phi_u_pos, um, phi_u_sum); break;
+        case 3: um_accumulate_kernel<3><<<grid, 128, 0, st>>>(m, s, G, first, phi_u_pos, um, phi_u_sum); break;
+        case 4: um_accumulate_kernel<4><<<grid, 128, 0, st>>>(m, s, G, first, phi_u_pos, um, phi_u_sum); break;
+        case 5: um_accumulate_kernel<5><<<grid, 128, 0, st>>>(m, s, G, first, phi_u_pos, um, phi_u_sum); break;
+        default: return cudaErrorInvalidValue;
+    }
     return cudaGetLastError();
 }
 

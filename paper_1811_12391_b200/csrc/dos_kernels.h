@@ -24,7 +24,12 @@ cudaError_t dos_launch_raytrace(const MeshDev &m, const SourceDev &s, const uint
 //                            sum_{g_lo<=g'<g} sig_s[m][l][g'->g] phi_all[g'][cell][lm]
 cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int G, int n_leg,
                                     int L, int g, int g_lo, const float *sig_s, const float *phi_u,
+                                    const float *um /* [G][Nv][MP] summed-source mode, else null */,
                                     const float *phi_all, float *qfix, cudaStream_t st);
+
+// summed-source mode: U^g[lm] (+)= Y_lm(Omega_p) phi_u,p^g, phi_u_sum^g (+)= phi_u,p^g after the ray trace of position p
+cudaError_t dos_launch_um_accumulate(const MeshDev &m, const SourceDev &s, int G, int L, int first, const float *phi_u_pos,
+                                     float *um, float *phi_u_sum, cudaStream_t st);
 
 // a4: Q = Q_fix + sig_s[m][l][g->g] phi (phi ignored when first != 0); phi = 0; also clears the sweep's
 // flags (n_flags ints at `done`) and its queue head.

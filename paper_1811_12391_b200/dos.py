@@ -20,7 +20,7 @@ DOS_OK = 0
 STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_ERR_STATE", -4: "DOS_ERR_NOMEM",
           -5: "DOS_ERR_CUDA", -6: "DOS_ERR_UNSUPPORTED"}
 
-EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_solve",
+EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_sum", "dos_solve",
            "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option", "dos_profile", "dos_profile_reset",
            "dos_sweep_trace_host",
            "dos_destroy", "dos_last_error"]
@@ -60,6 +60,8 @@ _lib.dos_set_material_host.restype = C.c_int
 _lib.dos_set_material_host.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dos_uncollided.restype = C.c_int
 _lib.dos_uncollided.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.dos_uncollided_sum.restype = C.c_int
+_lib.dos_uncollided_sum.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
 _lib.dos_solve.restype = C.c_int
 _lib.dos_solve.argtypes = [C.c_void_p, C.c_int32]
 _lib.dos_fluence.restype = C.c_int
@@ -146,7 +148,7 @@ def dos_workspace_bytes(mesh, sigma_t, sigma_s, kerma, quad, P_L, n_batch=1) -> 
 class Context:
     """Owner of one dos_ctx plus the torch tensors (workspace, material ids) it lives in."""
 
-    def __init__(self, mesh, material, sigma_t, sigma_s, kerma, quad, P_L, device="cuda:0", stream=None):
+    def __init__(self, mesh, material, sigma_t, sigma_s, kerma, quad, P_L, device="cuda:0", stream=None, n_batch=1):
         import torch
         self.torch = torch
         self.mesh = dict(mesh)
@@ -154,7 +156,7 @@ class Context:
         self.G = int(np.asarray(sigma_t).shape[1])
         self.shape = (mesh["nz"], mesh["ny"], mesh["nx"])
         self._tables = _Tables(sigma_t, sigma_s, kerma, quad)
-        nbytes = dos_workspace_bytes(mesh, sigma_t, sigma_s, kerma, quad, P_L)
+        nbytes = dos_workspace_bytes(mesh, sigma_t, sigma_s, kerma, quad, P_L, n_batch)
         self.workspace_bytes = nbytes
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
@@ -185,6 +187,12 @@ class Context:
         sp = _f32(spectrum)
         ptr = phi_u_out.data_ptr() if phi_u_out is not None else None
         self._check(_lib.dos_uncollided(self.handle, C.byref(src), sp.ctypes.data, ptr))
+
+    def dos_uncollided_sum(self, source, spectrum, first, phi_u_out=None):
+        src = _source_struct(source)
+        sp = _f32(spectrum)
+        ptr = phi_u_out.data_ptr() if phi_u_out is not None else None
+        self._check(_lib.dos_uncollided_sum(self.handle, C.byref(src), sp.ctypes.data, int(bool(first)), ptr))
 
     def dos_solve(self, n_iter):
         self._check(_lib.dos_solve(self.handle, int(n_iter)))
@@ -254,4 +262,25 @@ def run_problem(p, source_index=0, n_iter=None, device="cuda:0", ctx=None):
     out = {"phi_u": pu.cpu().numpy(), "phi_c": pc.cpu().numpy(), "phi_total": pt.cpu().numpy(), "dose": d.cpu().numpy()}
     if own:
         ctx.close()
+    return out
+
+
+def run_problem_summed(p, source_indices=None, n_iter=None, device="cuda:0"):
+    """Summed-source mode (dos_uncollided_sum): all the given source positions form ONE source, one solve.
+    Returns the same dict as run_problem (phi_u = the summed uncollided fluence)."""
+    idx = list(range(len(p["sources"]))) if source_indices is None else list(source_indices)
+    ctx = Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"],
+                  device=device, n_batch=max(2, len(idx)))
+    pu, pc, pt, d = ctx.new_field(), ctx.new_field(), ctx.new_field(), ctx.new_field(groups=False)
+    one = ctx.new_field()
+    pu.zero_()
+    for n, s in enumerate(idx):
+        ctx.dos_uncollided_sum(p["sources"][s], p["spectrum"], first=(n == 0), phi_u_out=one)
+        pu += one                                   # bookkeeping of the return value only; the library keeps its own sum
+    ctx.dos_solve(p["n_iter"] if n_iter is None else n_iter)
+    ctx.dos_fluence(pc, pt)
+    ctx.dos_dose(d, False)
+    ctx.dos_check()
+    out = {"phi_u": pu.cpu().numpy(), "phi_c": pc.cpu().numpy(), "phi_total": pt.cpu().numpy(), "dose": d.cpu().numpy()}
+    ctx.close()
     return out

@@ -74,9 +74,12 @@ def test_workspace_bytes_and_host_side_validation():
     with pytest.raises(dos.DosError) as e:
         dos.dos_workspace_bytes(bad, p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 1)
     assert e.value.status == -1
+    # n_batch > 1 adds the summed-source buffers: [G][Nv][MP] + [G][Nv] floats (MP = 4 at P1)
+    n2 = dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 1, n_batch=2)
+    assert n2 >= n + 4 * nv * p["n_group"] * (4 + 1)
     with pytest.raises(dos.DosError) as e:
-        dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 1, n_batch=2)
-    assert e.value.status == -6
+        dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], 1, n_batch=0)
+    assert e.value.status == -1
     q = {k: (v[:20] if k in ("mu", "eta", "xi", "w") else v) for k, v in p["quadrature"].items()}
     with pytest.raises(dos.DosError) as e:
         dos.dos_workspace_bytes(p["mesh"], p["sigma_t"], p["sigma_s"], p["kerma"], q, 1)

@@ -91,6 +91,41 @@ def test_every_sweep_variant_parity(dos, orc, case):
         ctx.close()
 
 
+def test_summed_source_mode_parity(dos, orc):
+    """several source positions as ONE source, one solve (dos_uncollided_sum)
+    against oracle.run_problem_summed; and the state machine of the mode."""
+    p = _make("config4", nx=30, ny=27, nz=7, voxel=1.3, n_group=5, n_iter=4, n_pos=5)
+    ref = orc.run_problem_summed(p, [0, 2, 3])
+    out = dos.run_problem_summed(p, [0, 2, 3])
+    assert_problem_parity(out, ref, "config4 small, positions 0+2+3 summed")
+    # one position through the summed path = the single-source path
+    one = dos.run_problem(p, source_index=1)
+    s1 = dos.run_problem_summed(p, [1])
+    for k in ("phi_u", "phi_total", "dose"):
+        assert np.abs(s1[k] - one[k]).max() <= 2e-6 * np.abs(one[k]).max(), k
+    # P5 (36 moments, tensor-core sweep) as well
+    p5 = _make("config3", nx=26, ny=20, nz=9, voxel=1.5, n_group=3, n_iter=3)
+    p5["sources"] = [p5["sources"][0], dict(p5["sources"][0], pos=np.array(p5["sources"][0]["pos"]) + np.array([9.0, 0.0, 2.0]))]
+    assert_problem_parity(dos.run_problem_summed(p5), orc.run_problem_summed(p5), "config3 small, 2 positions summed")
+    # a context without the summed-source buffers refuses the mode; first = 0 needs a first source
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_uncollided_sum(p["sources"][0], p["spectrum"], first=True)
+    assert e.value.status == -3
+    ctx.close()
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"], n_batch=2)
+    with pytest.raises(dos.DosError) as e:
+        ctx.dos_uncollided_sum(p["sources"][0], p["spectrum"], first=False)
+    assert e.value.status == -3
+    # a summed state is replaced by a later single-source call
+    ctx.dos_uncollided_sum(p["sources"][0], p["spectrum"], first=True)
+    ctx.dos_uncollided_sum(p["sources"][2], p["spectrum"], first=False)
+    out1 = dos.run_problem(p, source_index=1, ctx=ctx)
+    ctx.close()
+    for k in ("phi_total", "dose"):          # equal up to the order of the moment reductions
+        assert np.abs(out1[k] - one[k]).max() <= 2e-6 * np.abs(one[k]).max(), k
+
+
 def test_config2_full_parity(dos, orc):
     """BASELINE.json configs[1] at full size and full iteration count."""
     p = _make("config2")

@@ -366,6 +366,38 @@ def test_cylinder_mirror_symmetry(orc):
 
 
 # ------------------------------------------------------------------ (6) brute force 4^3 -----------
+def test_summed_source_reduces_to_single_source_and_is_linear_in_the_source(orc):
+    """oracle.run_problem_summed. Pins: (a) one position through the summed path
+    (external first-collision moments) equals the single-source path; (b) the same position given twice with half
+    the spectrum each equals the position given once -- the sum is formed before the (non-linear) fixup sees it;
+    (c) two positions mirrored in x on the x-symmetric cylinder give an x-symmetric dose; (d) the summed uncollided
+    fluence is the sum of the positions' own."""
+    p = make_problem("config2", nx=14, ny=12, nz=4, voxel=2.5, n_group=3, n_iter=3, sn=4, pl=2)
+    one = orc.run_problem(p)
+    a = orc.run_problem_summed(p, [0])
+    for k in ("phi_u", "phi_c", "phi_total", "dose"):
+        np.testing.assert_allclose(a[k], one[k], rtol=1e-12, atol=1e-300 + 1e-13 * np.abs(one[k]).max(), err_msg=k)
+    p2 = dict(p)
+    p2["sources"] = [p["sources"][0], p["sources"][0]]
+    p2["spectrum"] = (np.asarray(p["spectrum"], dtype=np.float64) / 2).astype(np.float32)    # halving is exact in fp32
+    b = orc.run_problem_summed(p2)
+    for k in ("phi_u", "phi_c", "dose"):
+        np.testing.assert_allclose(b[k], one[k], rtol=1e-12, atol=1e-13 * np.abs(one[k]).max(), err_msg=k)
+    s0 = p["sources"][0]
+    mir = {k: (np.array(v, dtype=np.float64) * np.array([-1.0, 1.0, 1.0]) if k in ("pos", "axis", "up") else v) for k, v in s0.items()}
+    p3 = dict(p)
+    p3["sources"] = [dict(s0, pos=np.array(s0["pos"]) + np.array([7.0, 0.0, 0.0])), None]
+    p3["sources"][1] = {k: (np.array(v, dtype=np.float64) * np.array([-1.0, 1.0, 1.0]) if k in ("pos", "axis", "up") else v)
+                        for k, v in p3["sources"][0].items()}
+    c = orc.run_problem_summed(p3)
+    assert np.abs(c["dose"]).max() > 0
+    np.testing.assert_allclose(c["dose"], c["dose"][:, :, ::-1], rtol=1e-9, atol=1e-12 * np.abs(c["dose"]).max())
+    u0 = orc.uncollided(p3["mesh"], p3["material"], p3["sigma_t"], p3["sources"][0], p3["spectrum"])
+    u1 = orc.uncollided(p3["mesh"], p3["material"], p3["sigma_t"], p3["sources"][1], p3["spectrum"])
+    np.testing.assert_allclose(c["phi_u"], u0 + u1, rtol=1e-14)
+    del mir
+
+
 def test_brute_force_linear_system_4cubed(orc):
     """north_star check 6: full linear system (cell-centre + face unknowns, DD closures, zero inflow,
     direct angle-to-angle P_l kernel of eq. 2) solved by sparse LU vs source iteration run to 1e-13."""
