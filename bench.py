@@ -178,11 +178,12 @@ def run_ours(args):
     nv = m["nx"] * m["ny"] * m["nz"]
     M = (p["P_L"] + 1) ** 2
     n_ang = len(p["quadrature"]["w"])
-    updates_per_step = n_updates(p)                      # this rank; all ranks do the same amount
+    summed = args.scan == "summed" and len(mine) > 1    # the positions form ONE source, one solve
+    updates_per_step = n_updates(p) // (len(mine) if summed else 1)   # this rank; all ranks do the same amount
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"],
-                          device=dev, stream=stream)
+                          device=dev, stream=stream, n_batch=len(mine) if summed else 1)
         dose = ctx.new_field(groups=False)
         flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
     ctx.dos_set_option("profile", 1)
@@ -190,7 +191,16 @@ def run_ours(args):
     dose_pinned = torch.empty(nv, dtype=torch.float32).pin_memory()
     mat_host, dose_host = mat_pinned.numpy(), dose_pinned.numpy().reshape(p["material"].shape)
 
+    def step_summed():
+        for n, s in enumerate(mine):
+            ctx.dos_uncollided_sum(p["sources"][s], p["spectrum"], first=(n == 0))
+        ctx.dos_solve(p["n_iter"])
+
     def step_device():
+        if summed:
+            step_summed()
+            ctx.dos_dose(dose, accumulate=False)
+            return
         for n, s in enumerate(mine):
             ctx.dos_uncollided(p["sources"][s], p["spectrum"])
             ctx.dos_solve(p["n_iter"])
@@ -198,6 +208,10 @@ def run_ours(args):
 
     def step_e2e():
         ctx.dos_set_material_host(mat_host)
+        if summed:
+            step_summed()
+            ctx.dos_dose_host(dose_host, accumulate=False)
+            return
         for n, s in enumerate(mine):
             ctx.dos_uncollided(p["sources"][s], p["spectrum"])
             ctx.dos_solve(p["n_iter"])
@@ -297,7 +311,8 @@ def run_ours(args):
             "metric": METRIC, "value": world * updates_per_step * args.steps / (total_ms * 1e-3), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "positions_per_rank": len(mine),
+            "config": {"workload": WORKLOADS[args.config] + (" -- summed-source mode: the positions form ONE source, one solve"
+                                                             if summed else ""), "positions_per_rank": len(mine),
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "flushed between timed steps (256 MiB fill)", "arithmetic": "fp32 sweep/sources/dose, fp64 ray trace"},
             "dose_map_ms": total_ms / args.steps, "phases_ms": phases, "wall_s_timed_region": wall,
@@ -337,6 +352,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="config2", choices=sorted(WORKLOADS))
     ap.add_argument("--positions", type=int, default=0, help="config4 only: source positions per step (default 36)")
+    ap.add_argument("--scan", default="separate", choices=["separate", "summed"],
+                    help="config4: one solve per source position with doses summed (default, BASELINE.json), or all "
+                         "positions as ONE source and one solve (the paper's CT-scan mode, PAPER.md:69-71)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
