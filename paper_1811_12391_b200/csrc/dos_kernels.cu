@@ -46,43 +46,33 @@ __global__ void __launch_bounds__(RT_THREADS) raytrace_kernel(MeshDev m, SourceD
     const double r = sqrt(r2);
     for (int t = 0; t < n_mat; ++t) s_len[t][threadIdx.x] = 0.0;
 
-    // walk from the centre (beta = 0) towards the source (beta = 1): direction e = s - c = -d
-    const double e[3] = {-dx, -dy, -dz};
-    const double c0[3] = {cx, cy, cz};
-    const double org[3] = {m.x0, m.y0, m.z0};
-    const double h[3] = {m.dx, m.dy, m.dz};
-    const int n[3] = {m.nx, m.ny, m.nz};
-    int idx[3] = {i, j, k};
-    int stp[3];
-    double inv[3], bnext[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        stp[a] = e[a] > 0.0 ? 1 : -1;
-        if (e[a] != 0.0) {
-            inv[a] = 1.0 / e[a];
-            const int plane = idx[a] + (e[a] > 0.0 ? 1 : 0);
-            bnext[a] = (org[a] + plane * h[a] - c0[a]) * inv[a];
-        } else {
-            inv[a] = 0.0;
-            bnext[a] = 1e300;
-        }
-    }
+    // Walk from the centre (beta = 0) towards the source (beta = 1): direction e = s - c = -d. Everything per axis
+    // lives in scalars and the axis of the next crossing is applied with selects: dynamically indexed arrays would
+    // sit in local memory (the first version: 160 bytes of stack, several local loads and stores per step).
+    // The next-crossing parameters advance by a constant per axis (fp64: <= 1e-13 after a few hundred steps).
+    const double ex = -dx, ey = -dy, ez = -dz;
+    const int sx = ex > 0.0 ? 1 : -1, sy = ey > 0.0 ? 1 : -1, sz = ez > 0.0 ? 1 : -1;
+    double bx = 1e300, by = 1e300, bz = 1e300, dbx = 0.0, dby = 0.0, dbz = 0.0;
+    if (ex != 0.0) { const double inv = 1.0 / ex; bx = (m.x0 + (i + (sx > 0 ? 1 : 0)) * m.dx - cx) * inv; dbx = fabs(m.dx * inv); }
+    if (ey != 0.0) { const double inv = 1.0 / ey; by = (m.y0 + (j + (sy > 0 ? 1 : 0)) * m.dy - cy) * inv; dby = fabs(m.dy * inv); }
+    if (ez != 0.0) { const double inv = 1.0 / ez; bz = (m.z0 + (k + (sz > 0 ? 1 : 0)) * m.dz - cz) * inv; dbz = fabs(m.dz * inv); }
+    int ix = i, iy = j, iz = k;
+    const long long px = sx, py = (long long)sy * m.nx, pz = (long long)sz * m.nx * m.ny;
     int cur = mat[cell];
     if (cur >= n_mat) { atomicExch(errflag, 1); cur = 0; }
     double run0 = 0.0;
-    const int sy = m.nx, sz = m.nx * m.ny;
-    size_t pos = cell;
+    long long pos = (long long)cell;
     for (;;) {
-        int a = 0;
-        double b = bnext[0];
-        if (bnext[1] < b) { b = bnext[1]; a = 1; }
-        if (bnext[2] < b) { b = bnext[2]; a = 2; }
+        const bool ax = bx <= by && bx <= bz, ay = !ax && by <= bz;          // ties: x, then y, then z
+        const double b = ax ? bx : (ay ? by : bz);
         if (b >= 1.0) { s_len[cur][threadIdx.x] += (1.0 - run0) * r; break; }      // source inside this cell
-        idx[a] += stp[a];
-        if (idx[a] < 0 || idx[a] >= n[a]) { s_len[cur][threadIdx.x] += (b - run0) * r; break; }   // left the mesh
-        pos += (ptrdiff_t)stp[a] * (a == 0 ? 1 : (a == 1 ? sy : sz));
-        const int plane = idx[a] + (stp[a] > 0 ? 1 : 0);
-        bnext[a] = (org[a] + plane * h[a] - c0[a]) * inv[a];
+        if (ax) { ix += sx; bx += dbx; pos += px; }
+        else if (ay) { iy += sy; by += dby; pos += py; }
+        else { iz += sz; bz += dbz; pos += pz; }
+        if ((unsigned)ix >= (unsigned)m.nx || (unsigned)iy >= (unsigned)m.ny || (unsigned)iz >= (unsigned)m.nz) {
+            s_len[cur][threadIdx.x] += (b - run0) * r;                              // left the mesh
+            break;
+        }
         int nm = mat[pos];
         if (nm >= n_mat) { atomicExch(errflag, 1); nm = 0; }
         if (nm != cur) {
