@@ -68,6 +68,9 @@ VARIANT_CASES = [
     ("config2", dict(nx=37, ny=21, nz=10, voxel=1.0, n_group=4, n_iter=4)),                        # S8/P3, ragged tiles
     ("config3", dict(nx=26, ny=20, nz=9, voxel=1.5, n_group=3, n_iter=3)),                         # S16/P5
     ("config2", dict(nx=33, ny=9, nz=5, voxel=1.1, n_group=3, n_iter=3, sn=6, pl=2)),              # S6/P2 (M padded 9->12)
+    ("config2", dict(nx=5, ny=3, nz=2, voxel=7.0, n_group=3, n_iter=2, sn=2, pl=0)),                # S2/P0: 1 angle, 1 moment
+    ("config1", {}),                                                                               # S4/P1, 16^3
+    ("config4", dict(nx=18, ny=16, nz=8, voxel=2.0, n_group=3, n_iter=3, n_pos=1, sn=12, pl=4)),   # S12/P4: 21 angles, 25 moments
 ]
 
 
