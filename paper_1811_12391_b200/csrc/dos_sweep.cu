@@ -75,12 +75,6 @@ __device__ __forceinline__ int lds_s32(unsigned a)
     asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
-__device__ __forceinline__ float4 lds_v4(unsigned a)
-{
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
-    return v;
-}
 __device__ __forceinline__ void sts_f32(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void sts_s32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
@@ -106,13 +100,6 @@ __device__ __forceinline__ void bar_compute(int n_threads) { asm volatile("bar.s
 __device__ __forceinline__ void st_release(int *p, int v)
 {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-__device__ __forceinline__ void red_add_v4(float *p, float4 v)
-{
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z),
-                 "f"(v.w)
-                 : "memory");
 }
 
 __device__ __forceinline__ void red_add_v2(float *p, float a, float b)
@@ -201,8 +188,8 @@ __device__ __forceinline__ void m2d_tiles(const float *qa, const float4 *bf, flo
 template <int MP, int I0, int N>
 __device__ __forceinline__ void d2m_tiles(const float *pa, const float4 *bf, int NA, float *r0, float *r1, bool on0, bool on1, int t4)
 {
-    if (N == 0) return;
-    float d[N > 0 ? N : 1][4];
+    if constexpr (N > 0) {
+    float d[N][4];
 #pragma unroll
     for (int i = 0; i < N; ++i) d[i][0] = d[i][1] = d[i][2] = d[i][3] = 0.f;
 #pragma unroll 1
@@ -211,10 +198,10 @@ __device__ __forceinline__ void d2m_tiles(const float *pa, const float4 *bf, int
         const float *p0 = pa + ka * 8 * PS;
         tf32_split_fast(p0[0], ah[0], al[0]); tf32_split_fast(p0[8], ah[1], al[1]);
         tf32_split_fast(p0[4 * PS], ah[2], al[2]); tf32_split_fast(p0[4 * PS + 8], ah[3], al[3]);
-        float4 b[N > 0 ? N : 1];
+        float4 b[N];
 #pragma unroll
         for (int i = 0; i < N; ++i) b[i] = bf[((I0 + i) * NA + ka) * 32];
-        mma_3xtf32<(N > 0 ? N : 1)>(d, ah, al, b);
+        mma_3xtf32<N>(d, ah, al, b);
     }
 #pragma unroll
     for (int i = 0; i < N; ++i)
@@ -222,6 +209,7 @@ __device__ __forceinline__ void d2m_tiles(const float *pa, const float4 *bf, int
             if (on0) red_add_v2(r0 + (I0 + i) * 8, d[i][0], d[i][1]);
             if (on1) red_add_v2(r1 + (I0 + i) * 8, d[i][2], d[i][3]);
         }
+    }
 }
 
 // 16-byte asynchronous global -> shared copy that bypasses L1 (tile faces are written by other SMs
