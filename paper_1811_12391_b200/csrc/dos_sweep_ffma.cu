@@ -137,23 +137,22 @@ __host__ __device__ constexpr int mps_of(int MP) { return ((MP / 4) & 1) ? MP : 
 
 // Slow path of the cell update: at least one extrapolated outflow was negative. Faces found negative
 // are pinned to zero together, the balance is re-solved, and the pinned set only grows (R12).
-// in/out: o = (psi_c, out_x, out_y, out_z) of the unfixed solve -> of the fixed one.
-__device__ __noinline__ float4 dd_fixup(float4 o, float q, float st, float cx, float cy, float cz, float ix, float iy,
-                                        float iz)
+// in/out: pc, ox, oy, oz of the unfixed solve -> of the fixed one.
+__device__ __forceinline__ void dd_fixup(float &pc, float &ox, float &oy, float &oz, float q, float st, float cx, float cy,
+                                         float cz, float ix, float iy, float iz)
 {
+    const float hx = cx * ix, hy = cy * iy, hz = cz * iz;
     bool fx = false, fy = false, fz = false;
-    for (;;) {
-        const bool ax = !fx && o.y < 0.f, ay = !fy && o.z < 0.f, az = !fz && o.w < 0.f;
-        if (!(ax || ay || az)) break;
-        fx |= ax; fy |= ay; fz |= az;
-        const float num = q + (fx ? 0.5f * cx : cx) * ix + (fy ? 0.5f * cy : cy) * iy + (fz ? 0.5f * cz : cz) * iz;
+#pragma unroll 1
+    do {
+        fx |= ox < 0.f; fy |= oy < 0.f; fz |= oz < 0.f;       // a pinned face's outflow is 0 and never tests negative
+        const float num = q + (fx ? 0.5f * hx : hx) + (fy ? 0.5f * hy : hy) + (fz ? 0.5f * hz : hz);
         const float den = st + (fx ? 0.f : cx) + (fy ? 0.f : cy) + (fz ? 0.f : cz);
-        o.x = num / den;
-        o.y = fx ? 0.f : 2.f * o.x - ix;
-        o.z = fy ? 0.f : 2.f * o.x - iy;
-        o.w = fz ? 0.f : 2.f * o.x - iz;
-    }
-    return o;
+        pc = __fdividef(num, den);
+        ox = fx ? 0.f : 2.f * pc - ix;
+        oy = fy ? 0.f : 2.f * pc - iy;
+        oz = fz ? 0.f : 2.f * pc - iz;
+    } while (fminf(ox, fminf(oy, oz)) < 0.f);
 }
 
 // One cp.async of 16 bytes that a thread issues every step: at step t it fetches what step s = t + dist
@@ -548,11 +547,8 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
                     const float num = fmaf(ccx[r], ix, fmaf(ccy[r], yin, fmaf(ccz[r], zin, q[r])));
                     pc = num * lds_f32(rd + 4 * r);
                     float ox = 2.f * pc - ix, oyr = 2.f * pc - yin, ozr = 2.f * pc - zin;
-                    if (fminf(ox, fminf(oyr, ozr)) < 0.f) {
-                        const float4 f = dd_fixup(make_float4(pc, ox, oyr, ozr), q[r], lds_f32(sig_a + 4 * m0), ccx[r], ccy[r],
-                                                  ccz[r], ix, yin, zin);
-                        pc = f.x; ox = f.y; oyr = f.z; ozr = f.w;
-                    }
+                    if (fminf(ox, fminf(oyr, ozr)) < 0.f)
+                        dd_fixup(pc, ox, oyr, ozr, q[r], lds_f32(sig_a + 4 * m0), ccx[r], ccy[r], ccz[r], ix, yin, zin);
                     px[r] = ox; oy[r] = oyr; oz[r] = ozr;
                     if (store_y) __stcg(fy_st + r * DOS_TK, oyr);
                     if (store_z) __stcg(fz_st + r * DOS_TJ, ozr);
