@@ -502,6 +502,228 @@ def test_moment_scatter_equals_direct_angle_sum(orc):
         assert np.abs(qn.ravel() - direct[nidx]).max() < 1e-13
 
 
+# ------------------------------------------------------------------ first-collision source, all l --
+def test_first_collision_equals_direct_legendre_kernel(orc):
+    """PAPER.md:49 (first-collision source) with eq. 2's scattering kernel (readings R2, R4): seen from
+    ordinate n, the source that uncollided photons arriving along Omega_r = (r_c - r_s)/r make in group g is
+        q_n = sum_l (2l+1) [sum_{g'<=g} sigma_sl^{g'->g} phi_u^{g'}] P_l(Omega_n . Omega_r)
+    (the angle-to-angle kernel applied to a delta function in angle). The moment-to-discrete of orc_first_collision's
+    output must reproduce it for every l <= L. A reversed Omega_r flips the odd l, a stray (2l+1) or a dropped g'
+    changes the sum: each fails here. P_l comes from numpy, Y_lm(Omega_n) from the pinned orc_harmonics."""
+    rng = np.random.default_rng(21)
+    L, G, n_leg = 3, 3, 4                                   # n_leg > L: the table holds more orders than are used
+    mesh = _mesh(4, 3, 2, 1.1, 0.9, 1.3)
+    mat = rng.integers(0, 2, size=(2, 3, 4)).astype(np.uint8)
+    sig_t = np.array([[0.3, 0.4, 0.5], [0.8, 0.9, 1.1]])
+    sig_s = np.zeros((2, n_leg + 1, G, G))
+    for gf in range(G):
+        for gt in range(gf, G):
+            sig_s[:, :, gf, gt] = rng.uniform(0.02, 0.2, size=(2, n_leg + 1)) * (0.6 ** np.arange(n_leg + 1))
+    pos = (6.1, -4.3, 2.2)                                   # generic direction: no component of Omega_r vanishes
+    spec = np.array([0.5, 0.3, 0.2])
+    pu = orc.uncollided(mesh, mat, sig_t, _iso_source(pos), spec)
+    M = (L + 1) ** 2
+    q = np.zeros((G, M, mat.size))
+    orc.first_collision(mesh, mat, sig_s, L, pos, pu, q)
+    Z, Y, X = _centres(mesh)
+    quad = quadrature.level_symmetric(6)
+    for n in (0, 7, 13, 22, 31, 40, 47):
+        om = np.array([quad["mu"][n], quad["eta"][n], quad["xi"][n]])
+        y = orc.harmonics(*om, L)
+        for (k, j, i) in [(0, 0, 0), (1, 2, 3), (0, 1, 2), (1, 0, 1)]:
+            cell = (k * 3 + j) * 4 + i
+            d = np.array([X[k, j, i] - pos[0], Y[k, j, i] - pos[1], Z[k, j, i] - pos[2]])
+            cosr = float(om @ d) / math.sqrt(float(d @ d))
+            for g in range(G):
+                got = sum((2 * l + 1) * y[l * (l + 1) + m] * q[g, l * (l + 1) + m, cell]
+                          for l in range(L + 1) for m in range(-l, l + 1))
+                want = sum((2 * l + 1) * _legendre_p(l, cosr) *
+                           sum(sig_s[mat[k, j, i], l, gp, g] * pu[gp, k, j, i] for gp in range(g + 1))
+                           for l in range(L + 1))
+                assert abs(got - want) <= 1e-13 * abs(want), (n, k, j, i, g)
+
+
+# ------------------------------------------------------------------ (6b) two groups, P1, brute force --
+def _dd_system_solve(n, h, mat, sig_t, sig_sl, quad, q_ang):
+    """Sparse LU of the full discrete system of ONE group on an n^3 mesh: unknowns are the cell-centre and face
+    angular fluxes of all ordinates; rows are the balance equation with the direct angle-to-angle P_l scattering
+    kernel of eq. 2, the three diamond closures per cell and zero inflow.
+    sig_sl [mat][l] in-group moments, q_ang [n_ang][n^3] fixed source per ordinate. Returns (psi [n_ang][n^3],
+    min face flux)."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+    na = len(quad["w"])
+    Om = np.stack([quad["mu"], quad["eta"], quad["xi"]], axis=1)
+    w = quad["w"]
+    cosm = Om @ Om.T
+    nl = sig_sl.shape[1]
+    nv = n ** 3
+    nfx = (n + 1) * n * n
+
+    def cid(i, j, k): return (k * n + j) * n + i
+    def fx(i, j, k): return (k * n + j) * (n + 1) + i
+    def fy(i, j, k): return (k * (n + 1) + j) * n + i
+    def fz(i, j, k): return (k * n + j) * n + i
+    per = nv + 3 * nfx
+    rows, cols, vals, rhs = [], [], [], []
+    def add(r, c, v): rows.append(r); cols.append(c); vals.append(v)
+    r = 0
+    for a in range(na):
+        base = a * per
+        off = (base + nv, base + nv + nfx, base + nv + 2 * nfx)
+        for k in range(n):
+            for j in range(n):
+                for i in range(n):
+                    c = cid(i, j, k)
+                    m = mat[k, j, i]
+                    lo = (off[0] + fx(i, j, k), off[1] + fy(i, j, k), off[2] + fz(i, j, k))
+                    hi = (off[0] + fx(i + 1, j, k), off[1] + fy(i, j + 1, k), off[2] + fz(i, j, k + 1))
+                    for d in range(3):
+                        add(r, hi[d], Om[a, d] / h[d]); add(r, lo[d], -Om[a, d] / h[d])
+                    add(r, base + c, sig_t[m])
+                    for b in range(na):
+                        kern = w[b] * sum((2 * l + 1) * sig_sl[m, l] * _legendre_p(l, cosm[a, b]) for l in range(nl))
+                        add(r, b * per + c, -kern)
+                    rhs.append(q_ang[a, c]); r += 1
+                    for d in range(3):
+                        add(r, base + c, 1.0); add(r, lo[d], -0.5); add(r, hi[d], -0.5)
+                        rhs.append(0.0); r += 1
+        for k in range(n):
+            for j in range(n):
+                add(r, off[0] + fx(0 if Om[a, 0] > 0 else n, j, k), 1.0); rhs.append(0.0); r += 1
+        for k in range(n):
+            for i in range(n):
+                add(r, off[1] + fy(i, 0 if Om[a, 1] > 0 else n, k), 1.0); rhs.append(0.0); r += 1
+        for j in range(n):
+            for i in range(n):
+                add(r, off[2] + fz(i, j, 0 if Om[a, 2] > 0 else n), 1.0); rhs.append(0.0); r += 1
+    assert r == na * per
+    A = sp.csc_matrix((vals, (rows, cols)), shape=(r, r))
+    sol = spla.spsolve(A, np.array(rhs))
+    psi = np.array([sol[a * per:a * per + nv] for a in range(na)])
+    faces = np.concatenate([sol[a * per + nv:(a + 1) * per] for a in range(na)])
+    return psi, faces.min()
+
+
+def test_brute_force_two_groups_p1_downscatter(orc):
+    """Eq. 2's g' sum for l >= 1: two groups, P1, sigma_s1^{0->1} != 0, and an ANISOTROPIC
+    source in group 0 so that group 0's l = 1 moments (and with them the l = 1 downscatter into group 1) are large.
+    Group by group the full linear system with the direct angle-to-angle kernel is solved by sparse LU; group 1's
+    fixed source is the direct double sum sum_n' w_n' sum_l (2l+1) sigma_sl^{0->1} P_l(Omega_n.Omega_n') psi_n'^{(0)}.
+    Source iteration run to convergence must agree in all four P1 moments of both groups. A cascade that used
+    sigma_s0 for every l (or dropped l >= 1, or mixed up from/to) fails."""
+    n = 4
+    h = (0.9, 1.0, 1.1)
+    mesh = _mesh(n, n, n, *h)
+    rng = np.random.default_rng(17)
+    mat = rng.integers(0, 2, size=(n, n, n)).astype(np.uint8)
+    sig_t = np.array([[0.30, 0.42], [0.45, 0.60]])                      # [mat][g]
+    sig_s = np.zeros((2, 2, 2, 2))                                      # [mat][l][from][to]
+    sig_s[0, 0] = [[0.08, 0.10], [0.0, 0.15]]
+    sig_s[0, 1] = [[0.03, 0.07], [0.0, 0.05]]
+    sig_s[1, 0] = [[0.12, 0.16], [0.0, 0.22]]
+    sig_s[1, 1] = [[0.05, 0.11], [0.0, 0.08]]
+    quad = quadrature.level_symmetric(4)
+    Om = np.stack([quad["mu"], quad["eta"], quad["xi"]], axis=1)
+    w = quad["w"]
+    cosm = Om @ Om.T
+    nv = n ** 3
+    # group 0 external source: Q00 + l = 1 moments (index order eta, xi, mu), q_n = Q00 + 3 (eta q1 + xi q2 + mu q3) > 0
+    Q00 = rng.uniform(0.9, 1.1, size=nv)
+    J = np.stack([0.20 * Q00, -0.12 * Q00, 0.15 * Q00])                 # moments lm = 1, 2, 3
+    q0_ang = np.array([Q00 + 3.0 * (Om[a, 1] * J[0] + Om[a, 2] * J[1] + Om[a, 0] * J[2]) for a in range(24)])
+    assert q0_ang.min() > 0
+    psi0, fmin0 = _dd_system_solve(n, h, mat, sig_t[:, 0], sig_s[:, :, 0, 0], quad, q0_ang)
+    # group 1: weak isotropic external source + downscatter from group 0 through the direct kernel
+    Q1 = 0.05 * rng.uniform(0.9, 1.1, size=nv)
+    mflat = mat.reshape(-1)
+    q1_ang = np.zeros((24, nv))
+    for a in range(24):
+        for b in range(24):
+            kern = w[b] * sum((2 * l + 1) * sig_s[mflat, l, 0, 1] * _legendre_p(l, cosm[a, b]) for l in range(2))
+            q1_ang[a] += kern * psi0[b]
+        q1_ang[a] += Q1
+    psi1, fmin1 = _dd_system_solve(n, h, mat, sig_t[:, 1], sig_s[:, :, 1, 1], quad, q1_ang)
+    assert min(psi0.min(), psi1.min()) > 0 and min(fmin0, fmin1) > -1e-14     # fixup inactive: SI solves the same system
+    qext = np.zeros((2, 4, nv))
+    qext[0, 0], qext[0, 1:4] = Q00, J
+    qext[1, 0] = Q1
+    phi = orc.solve(mesh, mat, sig_t, sig_s, quad, 1, 300, q_ext=qext.reshape(2, 4, n, n, n))
+    for g, psi in enumerate((psi0, psi1)):
+        bf = [(w[:, None] * psi).sum(0)] + [(w[:, None] * Om[:, d:d + 1] * psi).sum(0) for d in (1, 2, 0)]
+        for lm in range(4):
+            assert np.abs(phi[g, lm].ravel() - bf[lm]).max() < 1e-12 * np.abs(bf[0]).max(), (g, lm)
+    # the l = 1 downscatter matters at a level far above the tolerance (so a cascade that ignores l is caught)
+    cur1 = (w[:, None] * Om[:, 0:1] * psi1).sum(0)
+    assert np.abs(cur1).max() > 1e-3 * (w[:, None] * psi1).sum(0).max()
+
+
+# ------------------------------------------------------------------ fixup with several faces (R12) --
+def test_fixup_two_negative_outflows_hand_computed(orc):
+    """Reading R12: all faces whose extrapolated outflow is negative in a pass are pinned to zero together,
+    then the balance is re-solved: psi_c = (q + sum_pinned (c_d/2) psi_in,d + sum_free c_d psi_in,d) / (sigma_t + sum_free c_d).
+    2 x 2 x 1 mesh, S2 (one ordinate per octant, mu = eta = xi = 1/sqrt(3)); for the (+,+,+) ordinate cell (1,1) receives
+    the outflows of the two source cells (1,0) and (0,1) as x and y inflow, has no source and a thick absorber, so both
+    its x and y outflows extrapolate negative while z does not. Values typed out by hand below.
+    (Pinning the negative faces one per pass instead reaches the same state: pinning a face with 2 psi_c < psi_in lowers
+    psi_c -- psi_c' - psi_c = c_x (psi_c - psi_in/2) D / (D (D - c_x)) < 0 -- so every other negative outflow stays
+    negative and is pinned in a later pass; the two orders differ only in rounding.)"""
+    quad = quadrature.level_symmetric(2)
+    a = next(i for i in range(8) if quad["mu"][i] > 0 and quad["eta"][i] > 0 and quad["xi"][i] > 0)
+    mu = 1.0 / math.sqrt(3.0)
+    dx, dy, dz = 1.0, 0.8, 2.5
+    mesh = _mesh(2, 2, 1, dx, dy, dz)
+    cx, cy, cz = 2 * mu / dx, 2 * mu / dy, 2 * mu / dz
+    mat = np.array([[[0, 0], [0, 1]]], np.uint8)             # [k][j][i]: cell (i=1, j=1) is the absorber
+    sig = np.array([0.1, 9.0])
+    Q = np.zeros((1, 1, 2, 2))
+    Q[0, 0, 0, 1] = 2.0                                      # cell (i=1, j=0)
+    Q[0, 0, 1, 0] = 3.0                                      # cell (i=0, j=1)
+    _, psi = orc.sweep(mesh, mat, sig, quad, 0, Q, want_psi=True)
+    p = psi[a].reshape(2, 2)                                 # [j][i]
+    # cell (0,0): no source, vacuum inflow
+    assert p[0, 0] == 0.0
+    # source cells: vacuum inflow on every face (their upwind neighbour (0,0) sends 0), all outflows 2 psi_c > 0
+    p10 = 2.0 / (0.1 + cx + cy + cz)
+    p01 = 3.0 / (0.1 + cx + cy + cz)
+    assert abs(p[0, 1] - p10) < 1e-15 and abs(p[1, 0] - p01) < 1e-15
+    ix, iy = 2 * p01, 2 * p10                                # x inflow from (0,1), y inflow from (1,0)
+    first = (cx * ix + cy * iy) / (9.0 + cx + cy + cz)       # unfixed solve
+    assert 2 * first - ix < 0 and 2 * first - iy < 0 and 2 * first > 0       # x and y negative, z not
+    want = (0.5 * cx * ix + 0.5 * cy * iy) / (9.0 + cz)      # both pinned together, z still free
+    assert 2 * want >= 0
+    assert abs(p[1, 1] - want) < 1e-15
+    assert abs(want - first) > 1e-3 * first                  # the fixup changed the answer
+
+
+def test_fixup_second_pass_adds_a_face(orc):
+    """The pinned set only grows (R12): a cell whose first pass finds ONE negative outflow (x), and whose re-solve
+    then finds a second (y), ends with both pinned; z stays free. 2 x 2 x 1 mesh as above with unequal sources."""
+    quad = quadrature.level_symmetric(2)
+    a = next(i for i in range(8) if quad["mu"][i] > 0 and quad["eta"][i] > 0 and quad["xi"][i] > 0)
+    mu = 1.0 / math.sqrt(3.0)
+    dx, dy, dz = 1.0, 1.0, 4.0
+    mesh = _mesh(2, 2, 1, dx, dy, dz)
+    cx, cy, cz = 2 * mu / dx, 2 * mu / dy, 2 * mu / dz
+    mat = np.array([[[0, 0], [0, 1]]], np.uint8)
+    s11 = 5.0
+    sig = np.array([0.1, s11])
+    Q = np.zeros((1, 1, 2, 2))
+    Q[0, 0, 0, 1] = 1.5                                      # feeds the y inflow of (1,1)
+    Q[0, 0, 1, 0] = 4.0                                      # feeds the x inflow of (1,1)
+    _, psi = orc.sweep(mesh, mat, sig, quad, 0, Q, want_psi=True)
+    p = psi[a].reshape(2, 2)
+    den0 = 0.1 + cx + cy + cz
+    ix, iy = 2 * 4.0 / den0, 2 * 1.5 / den0
+    p1 = (cx * ix + cy * iy) / (s11 + cx + cy + cz)
+    assert 2 * p1 - ix < 0 and 2 * p1 - iy > 0               # pass 1: only x negative
+    p2 = (0.5 * cx * ix + cy * iy) / (s11 + cy + cz)
+    assert 2 * p2 - iy < 0                                   # pass 2: y turns negative
+    p3 = (0.5 * cx * ix + 0.5 * cy * iy) / (s11 + cz)
+    assert 2 * p3 >= 0
+    assert abs(p[1, 1] - p3) < 1e-15
+
+
 # ------------------------------------------------------------------ dose --------------------------
 def test_dose_linear_functional_and_air_zero(orc):
     """D = sum_g K[mat][g] (phi_u + phi_c00); air row of K = 0 => D = 0 in air."""
