@@ -16,6 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dos_oracle.c")
+_SRC_BLOCKED = os.path.join(_HERE, "dos_oracle_blocked.c")     # second loop arrangement, bit-identical (golden runs)
 _LIB = os.path.join(_HERE, "libdos_oracle.so")
 _lib = None
 
@@ -27,11 +28,17 @@ class _Mesh(C.Structure):
 
 
 def build(force: bool = False) -> str:
-    """gcc -O2 -fopenmp -shared; rebuilt when the source is newer than the library."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-                               "-o", _LIB, _SRC, "-lm"])
+    """gcc -O2 -fopenmp -shared; rebuilt when a source is newer than the library. -ffp-contract=off: no fused
+    multiply-add, so the two loop arrangements round identically; the vectoriser flags change no result."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_BLOCKED)):
+        subprocess.check_call(["gcc", "-O2", "-ftree-vectorize", "-fvect-cost-model=dynamic", "-std=c11", "-fopenmp", "-fPIC",
+                               "-shared", "-ffp-contract=off", "-o", _LIB, _SRC, _SRC_BLOCKED, "-lm"])
     return _LIB
+
+
+def source_files():
+    """The C sources whose text keys the stored golden results (tests/golden)."""
+    return [_SRC, _SRC_BLOCKED]
 
 
 def lib():
@@ -44,6 +51,8 @@ def lib():
         _lib.orc_first_collision.restype = None
         _lib.orc_sweep.restype = C.c_int
         _lib.orc_solve.restype = C.c_int
+        _lib.orc_solve_iters.restype = C.c_int
+        _lib.orc_solve_blocked.restype = C.c_int
         _lib.orc_dose.restype = None
     return _lib
 
@@ -142,10 +151,13 @@ def bnd_state_size(mesh, n_ang):
 
 
 def solve(mesh, material, sigma_t, sigma_s, quad, L, n_iter, source_pos=None, phi_u=None, q_ext=None,
-          reflective=False, want_balance=False, want_abs=False):
+          reflective=False, want_balance=False, want_abs=False, blocked=False, n_iter_g=None, want_conv=False):
     """Group cascade + source iteration. Returns phi_c moments [G][M][nz][ny][nx] (float64)
     (and, if want_balance, (leak[G], src_last[G]) of each group's last sweep; if want_abs, the
-    diagnostic sum_n w_n |psi_n| [G][nz][ny][nx] of each group's last sweep)."""
+    diagnostic sum_n w_n |psi_n| [G][nz][ny][nx] of each group's last sweep).
+    blocked=True runs dos_oracle_blocked.c, the bit-identical second loop arrangement (vacuum boundaries only).
+    n_iter_g [G] replaces n_iter group by group; want_conv appends each group's last-iteration stopping measure
+    max|phi00^(it) - phi00^(it-1)| / max|phi00^(it)| (the quantity dos_solve_tol tests) to the result."""
     sig_t, sig_s = _d(sigma_t), _d(sigma_s)
     n_mat, G = sig_t.shape
     n_leg = sig_s.shape[1] - 1
@@ -163,12 +175,26 @@ def solve(mesh, material, sigma_t, sigma_s, quad, L, n_iter, source_pos=None, ph
     pos = _d(source_pos) if source_pos is not None else np.zeros(3)
     pabs = np.zeros((G, nv)) if want_abs else None
     ms = _mesh(mesh)
-    rc = lib().orc_solve(C.byref(ms), _p(mat), C.c_int(n_mat), C.c_int(G), C.c_int(n_leg), C.c_int(L), _p(sig_t),
-                         _p(sig_s), C.c_int(n_ang), _p(mu), _p(eta), _p(xi), _p(w), _p(pos), _p(pu), _p(qe),
-                         C.c_int(n_iter), C.c_int(int(reflective)), _p(phi_c), _p(leak), _p(src), _p(pabs))
+    conv = None
+    if blocked:
+        if reflective or want_balance or want_conv or n_iter_g is not None:
+            raise ValueError("the blocked arrangement has vacuum boundaries and no balance outputs")
+        rc = lib().orc_solve_blocked(C.byref(ms), _p(mat), C.c_int(n_mat), C.c_int(G), C.c_int(n_leg), C.c_int(L),
+                                     _p(sig_t), _p(sig_s), C.c_int(n_ang), _p(mu), _p(eta), _p(xi), _p(w), _p(pos),
+                                     _p(pu), _p(qe), C.c_int(n_iter), _p(phi_c), _p(pabs))
+    else:
+        nig = np.ascontiguousarray(n_iter_g, dtype=np.int32) if n_iter_g is not None else None
+        assert nig is None or nig.shape == (G,)
+        conv = np.zeros(G) if want_conv else None
+        rc = lib().orc_solve_iters(C.byref(ms), _p(mat), C.c_int(n_mat), C.c_int(G), C.c_int(n_leg), C.c_int(L), _p(sig_t),
+                                   _p(sig_s), C.c_int(n_ang), _p(mu), _p(eta), _p(xi), _p(w), _p(pos), _p(pu), _p(qe),
+                                   C.c_int(n_iter), _p(nig), C.c_int(int(reflective)), _p(phi_c), _p(leak), _p(src),
+                                   _p(pabs), _p(conv))
     if rc:
         raise MemoryError("orc_solve")
     phi_c = phi_c.reshape((G, M) + mat.shape)
+    if want_conv:
+        return phi_c, conv
     if want_abs:
         return phi_c, pabs.reshape((G,) + mat.shape)
     return (phi_c, leak, src) if want_balance else phi_c
@@ -189,14 +215,15 @@ def dose(mesh, material, kerma, phi_u, phi_c_moments, dose_in=None):
     return tot.reshape((G,) + mat.shape), d.reshape(mat.shape)
 
 
-def run_problem(p, source_index=0, n_iter=None):
+def run_problem(p, source_index=0, n_iter=None, blocked=False):
     """Whole path O1-O5 for one source position of a problem dict from inputs.make_problem.
     Returns dict(phi_u, phi_c (scalar, [G][nz][ny][nx]), phi_total, dose, phi_c_moments, phi_c_abs
     (sum_n w_n |psi_n| of each group's last sweep: the parity tests' conditioning scale))."""
     src = p["sources"][source_index]
     pu = uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
     pc, pabs = solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"],
-                     p["n_iter"] if n_iter is None else n_iter, source_pos=src["pos"], phi_u=pu, want_abs=True)
+                     p["n_iter"] if n_iter is None else n_iter, source_pos=src["pos"], phi_u=pu, want_abs=True,
+                     blocked=blocked)
     tot, d = dose(p["mesh"], p["material"], p["kerma"], pu, pc)
     return {"phi_u": pu, "phi_c": pc[:, 0], "phi_total": tot, "dose": d, "phi_c_moments": pc, "phi_c_abs": pabs}
 

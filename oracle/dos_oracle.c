@@ -264,8 +264,9 @@ void orc_first_collision(const orc_mesh *ms, const uint8_t *mat, int G, int n_le
 
 /* --------------------------------------------------------------------- O4 one sweep ----------- */
 /* Cell update: diamond difference with set-to-zero fixup WITH rebalance (reading R3, R12).
- * psi_in[3], c[3] = 2|Omega_d|/Delta_d, returns psi_c, writes psi_out[3]. */
-static double dd_cell(double q, double sig_t, const double c[3], const double pin[3], double pout[3])
+ * psi_in[3], c[3] = 2|Omega_d|/Delta_d, returns psi_c, writes psi_out[3]. (Not static: dos_oracle_blocked.c, the
+ * second loop arrangement used for full-size golden runs, calls this same function.) */
+double orc_dd_cell(double q, double sig_t, const double c[3], const double pin[3], double pout[3])
 {
     int fixed[3] = {0, 0, 0};
     double pc = 0.0;
@@ -321,7 +322,7 @@ static void sweep_angle(const orc_mesh *ms, const uint8_t *mat, const double *si
                 double q = 0.0;
                 for (int lm = 0; lm < M; ++lm) q += coef[lm] * Q[(size_t)lm * nv + cell];
                 double pin[3] = {fx, fy[i], fz[(size_t)j * nx + i]}, pout[3];
-                psi_c[cell] = dd_cell(q, sig_t_g[mat[cell]], c, pin, pout);
+                psi_c[cell] = orc_dd_cell(q, sig_t_g[mat[cell]], c, pin, pout);
                 fx = pout[0];
                 fy[i] = pout[1];
                 fz[(size_t)j * nx + i] = pout[2];
@@ -436,11 +437,14 @@ int orc_sweep(const orc_mesh *ms, const uint8_t *mat, const double *sig_t_g, int
  * phi_c out [G][M][Nv]. leak out [G] (may be NULL): leakage of the LAST sweep of each group.
  * absorbed-source bookkeeping for the balance pin: src_last [G] (may be NULL) = sum_c V Q[00](c) of
  * the last sweep's source. phi_abs [G][Nv] (may be NULL): orc_sweep's diagnostic of the last sweep. */
-int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_leg, int L,
-              const double *sigma_t, const double *sigma_s, int n_ang, const double *mu,
-              const double *eta, const double *xi, const double *w, const double *pos,
-              const double *phi_u, const double *q_ext, int n_iter, int reflective, double *phi_c,
-              double *leak, double *src_last, double *phi_abs)
+/* n_iter_g (may be NULL): per-group iteration counts that replace n_iter (the counts a tolerance-stopped GPU run
+ * reports, so that both sides do the same number of sweeps). conv out [G] (may be NULL): the
+ * stopping measure of the last iteration of each group, max_c |phi00^(it) - phi00^(it-1)| / max_c |phi00^(it)|. */
+int orc_solve_iters(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_leg, int L,
+                    const double *sigma_t, const double *sigma_s, int n_ang, const double *mu,
+                    const double *eta, const double *xi, const double *w, const double *pos,
+                    const double *phi_u, const double *q_ext, int n_iter, const int *n_iter_g, int reflective,
+                    double *phi_c, double *leak, double *src_last, double *phi_abs, double *conv)
 {
     size_t nv = (size_t)ms->nx * ms->ny * ms->nz, nb = bnd_size(ms);
     int M = (L + 1) * (L + 1);
@@ -468,7 +472,8 @@ int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_le
         double *phi = phi_c + (size_t)g * M * nv;
         memset(phi_old, 0, sizeof(double) * (size_t)M * nv);
         if (bnd) memset(bnd, 0, sizeof(double) * (size_t)n_ang * nb);
-        for (int it = 1; it <= n_iter && rc == 0; ++it) {
+        const int n_it = n_iter_g ? n_iter_g[g] : n_iter;
+        for (int it = 1; it <= n_it && rc == 0; ++it) {
             for (int l = 0; l <= L; ++l)
                 for (int mm = -l; mm <= l; ++mm) {
                     int lm = l * (l + 1) + mm;
@@ -476,7 +481,7 @@ int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_le
                         q[(size_t)lm * nv + c] = qfix[(size_t)lm * nv + c] +
                             sigma_s[(((size_t)mat[c] * (n_leg + 1) + l) * G + g) * G + g] * phi_old[(size_t)lm * nv + c];
                 }
-            int last = (it == n_iter);
+            int last = (it == n_it);
             rc = orc_sweep(ms, mat, sig_t_g, n_ang, mu, eta, xi, w, L, q, phi, reflective, bnd,
                            (leak && last) ? &leak[g] : NULL, NULL,
                            (phi_abs && last) ? phi_abs + (size_t)g * nv : NULL);
@@ -485,11 +490,31 @@ int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_le
                 for (size_t c = 0; c < nv; ++c) s += q[c];
                 src_last[g] = s * ms->dx * ms->dy * ms->dz;
             }
+            if (last && conv) {
+                double dmax = 0.0, pmax = 0.0;
+                for (size_t c = 0; c < nv; ++c) {
+                    double d = fabs(phi[c] - phi_old[c]), a = fabs(phi[c]);
+                    if (d > dmax) dmax = d;
+                    if (a > pmax) pmax = a;
+                }
+                conv[g] = pmax > 0.0 ? dmax / pmax : 0.0;
+            }
             memcpy(phi_old, phi, sizeof(double) * (size_t)M * nv);
         }
     }
     free(qfix); free(q); free(phi_old); free(sig_t_g); free(bnd);
     return rc;
+}
+
+/* The fixed-count form every config uses (reading R5): n_iter sweeps in every group, no convergence test. */
+int orc_solve(const orc_mesh *ms, const uint8_t *mat, int n_mat, int G, int n_leg, int L,
+              const double *sigma_t, const double *sigma_s, int n_ang, const double *mu,
+              const double *eta, const double *xi, const double *w, const double *pos,
+              const double *phi_u, const double *q_ext, int n_iter, int reflective, double *phi_c,
+              double *leak, double *src_last, double *phi_abs)
+{
+    return orc_solve_iters(ms, mat, n_mat, G, n_leg, L, sigma_t, sigma_s, n_ang, mu, eta, xi, w, pos, phi_u, q_ext,
+                           n_iter, NULL, reflective, phi_c, leak, src_last, phi_abs, NULL);
 }
 
 /* ------------------------------------------------------------------ O5 totals and dose -------- */

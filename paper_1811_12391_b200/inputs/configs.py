@@ -37,7 +37,10 @@ _SPECS = {
 
 def make_problem(name: str, **override):
     """Build a workload. `override` may replace nx, ny, nz, voxel, n_group, sn, pl, n_iter (for reduced
-    parity cases that keep the structure of a config at a size the oracle finishes in seconds)."""
+    parity cases that keep the structure of a config at a size the oracle finishes in seconds).
+    `top_groups=k` keeps only the k highest-energy groups of the config's own group structure (tables and spectrum
+    cut, not re-generated or re-normalised): photons only downscatter, so groups 0..k-1 of the full problem ARE
+    this problem, and a parity run of it is a parity run of the head of the full cascade."""
     nx, ny, nz, vox, n_group, sn, pl, n_iter, kind, n_pos = _SPECS[name]
     nx = override.get("nx", nx); ny = override.get("ny", ny); nz = override.get("nz", nz)
     vox = override.get("voxel", vox); n_group = override.get("n_group", n_group)
@@ -68,6 +71,13 @@ def make_problem(name: str, **override):
             sources = [scan_source(2.0 * math.pi * 9 / 36)]
         else:
             sources = [scan_source(2.0 * math.pi * p / n_pos) for p in range(n_pos)]
+    top = override.get("top_groups")
+    if top is not None and top < n_group:
+        table = {"sigma_t": np.ascontiguousarray(table["sigma_t"][:, :top]),
+                 "sigma_s": np.ascontiguousarray(table["sigma_s"][:, :, :top, :top]),
+                 "kerma": np.ascontiguousarray(table["kerma"][:, :top]), "edges": table["edges"][:top + 1]}
+        spectrum = np.ascontiguousarray(spectrum[:top])
+        n_group = top
     return {"name": name, "mesh": mesh, "material": mat, "materials": mats,
             "sigma_t": table["sigma_t"], "sigma_s": table["sigma_s"], "kerma": table["kerma"],
             "edges": table["edges"], "n_group": n_group, "n_leg": pl, "P_L": pl, "quadrature": quad,

@@ -724,6 +724,86 @@ def test_fixup_second_pass_adds_a_face(orc):
     assert abs(p[1, 1] - p3) < 1e-15
 
 
+# ------------------------------------------------------------------ iteration counts, stopping measure --
+def test_per_group_iteration_counts_and_stopping_measure(orc):
+    """orc_solve_iters: (a) per-group counts all equal to n reproduce the fixed-count solve bit for
+    bit; (b) one cell, P0, vacuum, isotropic source, in-group scattering: phi^(k) = A (Q + sigma_s phi^(k-1)) with
+    A = sum_n w_n / (sigma_t + cx + cy + cz) (the single-cell closed form above), a geometric series of ratio
+    r = A sigma_s, so the stopping measure after k sweeps is |phi^k - phi^(k-1)| / phi^k = r^(k-1) / sum_{j<k} r^j;
+    (c) a group given fewer sweeps stops earlier: its fluence equals the fixed-count solve with that count."""
+    p = make_problem("config1", nx=5, ny=4, nz=3, n_iter=4)
+    src = p["sources"][0]
+    pu = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+    args = (p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], 1)
+    a = orc.solve(*args, 4, source_pos=src["pos"], phi_u=pu)
+    b = orc.solve(*args, 99, source_pos=src["pos"], phi_u=pu, n_iter_g=[4, 4, 4, 4])
+    assert np.array_equal(a, b)
+    c = orc.solve(*args, 99, source_pos=src["pos"], phi_u=pu, n_iter_g=[2, 4, 4, 4])
+    two = orc.solve(*args, 2, source_pos=src["pos"], phi_u=pu)
+    assert np.array_equal(c[0], two[0]) and not np.array_equal(c[0], a[0])
+    # (b)
+    quad = quadrature.level_symmetric(4)
+    mesh = _mesh(1, 1, 1, 0.8, 1.1, 1.7)
+    sig_t, sig_s0 = 0.9, 0.6
+    A = (quad["w"] / (sig_t + 2 * np.abs(quad["mu"]) / 0.8 + 2 * np.abs(quad["eta"]) / 1.1 + 2 * np.abs(quad["xi"]) / 1.7)).sum()
+    r = A * sig_s0
+    qext = np.zeros((1, 1, 1, 1, 1))
+    qext[0, 0] = 1.7
+    ss = np.full((1, 1, 1, 1), sig_s0)
+    for k in (1, 2, 5, 9):
+        phi, conv = orc.solve(mesh, np.zeros((1, 1, 1), np.uint8), np.array([[sig_t]]), ss, quad, 0, k, q_ext=qext,
+                              want_conv=True)
+        series = sum(r ** j for j in range(k))
+        assert abs(phi[0, 0, 0, 0, 0] - 1.7 * A * series) < 1e-14
+        assert abs(conv[0] - r ** (k - 1) / series) < 1e-13
+
+
+# ------------------------------------------------------------------ second loop arrangement, goldens --
+@pytest.mark.parametrize("name,ov", [
+    ("config1", {}),
+    ("config2", dict(nx=21, ny=13, nz=6, voxel=1.8, n_group=5, n_iter=3)),                     # S8/P3
+    ("config3", dict(nx=18, ny=11, nz=7, voxel=2.0, n_group=4, n_iter=3)),                     # S16/P5
+    ("config4", dict(nx=17, ny=15, nz=5, voxel=2.2, n_group=5, n_iter=3, n_pos=1)),            # 5 materials
+    ("config2", dict(nx=9, ny=5, nz=3, voxel=4.0, n_group=3, n_iter=2, sn=6, pl=2)),
+])
+def test_blocked_variant_is_bit_identical(orc, name, ov):
+    """dos_oracle_blocked.c (used by tests/golden/make_golden.py for the full-size runs) re-arranges the loops of
+    orc_solve; every output must equal the plain nested-loop oracle's bit for bit, whatever the thread count."""
+    p = make_problem(name, **ov)
+    a = orc.run_problem(p)
+    b = orc.run_problem(p, blocked=True)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_golden_files_match_inputs_and_oracle_source(orc):
+    """Every stored result under tests/golden/ is keyed by a hash of its problem's inputs and of oracle/*.c; a stale
+    file (inputs or oracle changed since it was written) fails here, before any GPU test trusts it. The small
+    self-test case is re-run and must reproduce its stored values exactly (the writer is deterministic and the
+    stored numbers are the oracle's)."""
+    import glob
+    import os
+    import sys
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    sys.path.insert(0, here)
+    import make_golden as mg
+    files = sorted(glob.glob(os.path.join(here, "*.npz")))
+    assert any(f.endswith("selftest.npz") for f in files)
+    for f in files:
+        case = os.path.basename(f)[:-4]
+        z = np.load(f)
+        config, ov, sidx, _ = mg.CASES[case]
+        p = make_problem(config, **ov)
+        assert str(z["key"]) == mg.problem_key(p, sidx), f"{case}: stale golden file, re-run tests/golden/make_golden.py {case}"
+        assert z["phi_c"].shape == (p["n_group"], z["cells"].size)
+    import tempfile
+    with tempfile.TemporaryDirectory() as tmp:
+        z0, z1 = np.load(os.path.join(here, "selftest.npz")), np.load(mg.make("selftest", out_dir=tmp))
+        for k in z0.files:
+            if k != "meta":
+                assert np.array_equal(z0[k], z1[k]), k
+
+
 # ------------------------------------------------------------------ dose --------------------------
 def test_dose_linear_functional_and_air_zero(orc):
     """D = sum_g K[mat][g] (phi_u + phi_c00); air row of K = 0 => D = 0 in air."""
