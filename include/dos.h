@@ -10,7 +10,9 @@
  *     The library never allocates device memory: all of its state lives in the caller's workspace,
  *     which must stay alive and untouched until dos_destroy.
  *   - Every call only ENQUEUES work on the CUDA stream given to dos_create (no host sync), except
- *     the *_host entry points, which synchronise that stream before returning.
+ *     dos_create itself, the *_host entry points that copy OUT (dos_dose_host), dos_check and dos_profile*, which
+ *     synchronise that stream before returning. Small host arguments (source, spectrum) are passed to the kernels by
+ *     value, so they may be freed as soon as the call returns.
  *   - Fields are [..][nz][ny][nx], x fastest. Group index 0 is the HIGHEST energy.
  *   - Errors: a negative dos_status, never an exception; text via dos_last_error().
  *   - Call order: dos_create -> dos_uncollided -> dos_solve -> dos_fluence / dos_dose (any order,
@@ -91,8 +93,10 @@ dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs, const dos
  * discrete-to-moment matrices ((2l+1) Y_lm(Omega_n) and w_n Y_lm(Omega_n); real Schmidt
  * semi-normalised harmonics, (P_L+1)^2 moments; readings R2, R10) and the diamond-difference
  * constants 2|Omega_d|/Delta_d, and lays out the workspace.
- *   d_material_ids  device uint8 [nz][ny][nx], values < n_mat (checked on the device at the first
- *                   dos_uncollided); caller-owned, must outlive the context
+ *   d_material_ids  device uint8 [nz][ny][nx], values < n_mat: the whole grid is checked on the device here (and again
+ *                   by dos_set_material_host); an id >= n_mat is reported by dos_check / dos_dose_host as
+ *                   DOS_ERR_INVALID_ARG, and every kernel clamps the id it indexes a table with, so a bad grid gives a
+ *                   flagged, wrong result, never an out-of-bounds access; caller-owned, must outlive the context
  *   P_L             scattering order used, 0 <= P_L <= min(xs->n_leg, 5)
  *   d_workspace     device, >= dos_workspace_bytes, 256-byte aligned
  *   cuda_stream     a cudaStream_t (NULL = legacy default stream)                                  */
@@ -101,7 +105,9 @@ dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint8_t *d_mate
                       size_t workspace_bytes, void *cuda_stream);
 
 /* Replace the material grid from HOST memory (copied into the workspace; the context then uses that
- * copy instead of d_material_ids). Used by the end-to-end path. */
+ * copy instead of d_material_ids) and check it (as dos_create does; the bad-id flag of the previous grid is cleared).
+ * Used by the end-to-end path. The copy is only enqueued: pageable memory is staged by the CUDA runtime before the
+ * call returns; PINNED memory must stay untouched until the stream has passed this point. */
 dos_status dos_set_material_host(dos_ctx *ctx, const uint8_t *h_material_ids);
 
 /* Uncollided fluence by ray tracing (readings R6-R9): for every voxel centre inside
@@ -124,6 +130,10 @@ dos_status dos_uncollided(dos_ctx *ctx, const dos_source *source, const float *s
  * Needs a workspace sized by dos_workspace_bytes with n_batch > 1 (else DOS_ERR_STATE). */
 dos_status dos_uncollided_sum(dos_ctx *ctx, const dos_source *source, const float *spectrum, int32_t first,
                               float *d_phi_u_out);
+
+/* The uncollided fluence the context currently holds -- of the last dos_uncollided, or the running sum over the
+ * positions given to dos_uncollided_sum since first != 0 -- copied to device [G][nz][ny][nx]. */
+dos_status dos_uncollided_total(dos_ctx *ctx, float *d_phi_u_out);
 
 /* Collided fluence (PAPER.md:39-45 eq. 2-3, :49): for g = 0..G-1, top-down (downscatter only):
  *   Q_fix = first-collision source moments Y_lm(Omega_r) sum_{g'<=g} sigma_sl^{g'->g} phi_u^{g'}
@@ -149,18 +159,14 @@ dos_status dos_dose_host(dos_ctx *ctx, float *h_dose, int32_t accumulate);
  * a material id >= n_mat (DOS_ERR_INVALID_ARG), a stuck sweep hand-off or a CUDA fault (DOS_ERR_CUDA). */
 dos_status dos_check(dos_ctx *ctx);
 
-/* Tuning / measurement knobs (all optional).
+/* Tuning / measurement knobs (all optional, all per context).
+ *   "sweep_contraction"  where the sweep's moment-to-discrete / discrete-to-moment contractions run: 0 (default) the
+ *                   tensor-memory sweep (tcgen05.mma kind::tf32, 3xTF32 split; dos_sweep_umma.cu) wherever the quadrature
+ *                   admits it and the FFMA sweep (dos_sweep_ffma.cu) otherwise; 1 FFMA; 2 tensor memory
  *   "sweep_chunk"   steps along x between face-flux hand-off publications of neighbouring tiles (>= 1)
  *   "sweep_grid"    number of persistent sweep CTAs
- *   "sweep_angles_per_warp", "sweep_aux_warps", "sweep_angle_split"  shape of the sweep CTA and number of
- *                   CTAs an octant's angles are spread over (0 = library default)
- *   "sweep_contraction"  where the sweep's moment-to-discrete / discrete-to-moment contractions run: 0 (default)
- *                   tensor cores (3xTF32 mma.sync) from P4 up and FFMA below, 1 FFMA, 2 tensor cores
- *   "sweep_two_per_sm"  bit 0: tensor-core sweep, bit 1: FFMA sweep (default 2). Where set, problems of <= 16
- *                   moments per cell use a sweep variant capped at 64 registers so that two CTAs share an SM (FFMA
- *                   sweep: only with >= 4 work items per SM). Process-wide.
- *   "sweep_impl"    0: dos_sweep.cu (default), 1: the first version kept for A/B measurements
- *   "sweep_trace_item"  see dos_sweep_trace_host
+ *   "sweep_angles_per_warp", "sweep_aux_warps", "sweep_angle_split", "sweep_two_per_sm"  shape of the FFMA sweep CTA
+ *                   (0 = library default)
  *   "profile"       1: bracket every sweep and ray-trace launch with CUDA events (see dos_profile)  */
 dos_status dos_set_option(dos_ctx *ctx, const char *name, int64_t value);
 
@@ -175,14 +181,6 @@ typedef struct {
 } dos_profile_t;
 dos_status dos_profile(dos_ctx *ctx, dos_profile_t *out);
 dos_status dos_profile_reset(dos_ctx *ctx);
-
-/* Diagnostic timeline of one sweep work item (option "sweep_trace_item" = (octant * ntk + tk) * ntj + tj, -1 =
- * off): after a dos_solve, copies to HOST the SM clock at which every warp of that item's CTA started each step
- * (k = 0), finished its first phase (1: staging copies for aux warps, moment-to-discrete for compute warps), its
- * second phase (2: discrete-to-moment / diamond difference) and reached the step's barrier (3), in the last
- * sweep launched: h_trace[(step * 32 + warp) * 4 + k], step < nx + 10, n = number of int64 to copy.
- * Synchronises the stream. */
-dos_status dos_sweep_trace_host(dos_ctx *ctx, int64_t *h_trace, size_t n);
 
 void dos_destroy(dos_ctx *ctx);
 

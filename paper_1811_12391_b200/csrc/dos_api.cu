@@ -1,6 +1,7 @@
 // dos_api.cu -- the C ABI of include/dos.h: context, validation, workspace layout, host-side tables,
-// and the launch sequence of the hot path. Kernels: dos_kernels.cu (ray trace, sources, dose) and
-// dos_sweep.cu (transport sweep). No code is shared with oracle/.
+// and the launch sequence of the hot path. Kernels: dos_kernels.cu (ray trace, sources, dose),
+// dos_sweep_umma.cu (transport sweep on the tensor-memory path) and dos_sweep_ffma.cu (its FFMA fallback).
+// No code is shared with oracle/.
 #include "../../include/dos.h"
 #include "dos_internal.h"
 #include "dos_kernels.h"
@@ -14,21 +15,20 @@
 #include <vector>
 
 struct Layout {
-    size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
-        spectrum, errflag, trace, um, phi_u_sum, total;
+    size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, items_u, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
+        bm2d, bd2m, signs, errflag, um, phi_u_sum, total;
 };
 
 struct dos_ctx {
     dos_mesh mesh;
     int n_mat, G, n_leg, L, M, MP, n_ang, per_oct;
-    int ntj, ntk, n_items, ag, n_grp, chunk, grid;     // ag/n_grp/chunk/grid: sweep (dos_sweep.cu)
-    int n_aux;                                         // aux warps of the sweep CTA
+    int ntj, ntk, n_items, ag, n_grp, chunk, grid;     // FFMA sweep: (octant, tile) items, angles per warp, warps, flag chunk, CTAs
+    int n_aux;                                         // aux warps of the FFMA sweep CTA
     int asplit, ag_pref, aux_pref;                     // angle split of an octant over CTAs; option overrides (0 = default)
-    int trace_item;                                    // sweep work item whose timeline is recorded, or -1
-    int contraction_pref;                              // 0 auto, 1 FFMA (dos_sweep_ffma.cu), 2 tensor cores (dos_sweep.cu)
-    bool mma;                                          // the choice in force
-    int impl;                                          // 0: dos_sweep.cu, 1: dos_sweep_v1.cu
-    int ag1, n_grp1, chunk1, grid1;                    // the same for the first version
+    int contraction_pref;                              // 0 auto, 1 FFMA (dos_sweep_ffma.cu), 2 tensor memory (dos_sweep_umma.cu)
+    bool umma, umma_ok;                                // the choice in force; the quadrature admits the tensor-memory sweep
+    int n_items_u, grid_u;                             // tensor-memory sweep: (quad, tile) items, CTAs
+    int two_per_sm;                                    // FFMA sweep: 64-register two-CTAs-per-SM variant (0 never, 1 from 4 items per SM, 2 always)
     size_t nv;
     cudaStream_t stream;
     const uint8_t *d_mat;        // current material grid (caller's or the workspace copy)
@@ -39,6 +39,7 @@ struct dos_ctx {
     bool can_sum, summed;        // workspace holds the summed-source buffers; the current uncollided state is a sum
     dos_source src;
     bool have_dose_acc;
+    bool mat_checked;            // the current material grid has been through validate_material_kernel
     bool profile, prof_open;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop); kind in ev_kind
     std::vector<int> ev_kind;     // 0 sweep, 1 ray trace
@@ -102,23 +103,22 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     const size_t nv = (size_t)m->nx * m->ny * m->nz;
     const int MP = dos_mpad(L), per = n_ang / 8;
     const int ntj = (m->ny + DOS_TJ - 1) / DOS_TJ, ntk = (m->nz + DOS_TK - 1) / DOS_TK;
-    const int ag1 = dos_sweep_v1_angles_per_warp(per, L);
-    const int n_grp1 = ag1 ? per / ag1 : 1;
-    // tile-face buffers: the larger of the two sweep versions' layouts
-    const size_t fy_v1 = (size_t)n_ang * ntj * m->nz * m->nx, fz_v1 = (size_t)n_ang * ntk * m->ny * m->nx;
-    const size_t fy_v2 = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK;
-    const size_t fz_v2 = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TJ;
+    const int KP = (MP + 7) & ~7, A8 = (per + 7) & ~7, NAP = (per + 15) & ~15, NMP = (MP + 15) & ~15;
+    // tile-face buffers, one per (octant, tile), indexed by wavefront diagonal
+    const size_t fy = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK;
+    const size_t fz = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TJ;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     l.phi_u = take(sizeof(float) * G * nv);
     l.phi_all = take(sizeof(float) * G * nv * MP);
     l.qfix = take(sizeof(float) * nv * MP);
     l.q = take(sizeof(float) * nv * MP);
-    l.fy = take(sizeof(float) * (fy_v1 > fy_v2 ? fy_v1 : fy_v2));
-    l.fz = take(sizeof(float) * (fz_v1 > fz_v2 ? fz_v1 : fz_v2));
-    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * (n_grp1 > 8 ? n_grp1 : 8));   // v2: up to 8 angle parts per tile
+    l.fy = take(sizeof(float) * fy);
+    l.fz = take(sizeof(float) * fz);
+    l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * 8);      // FFMA sweep: up to 8 angle parts per (octant, tile)
     l.queue = take(sizeof(int) * 4);
     l.items = take(sizeof(int) * (size_t)8 * ntj * ntk);
+    l.items_u = take(sizeof(int) * (size_t)2 * ntj * ntk);
     l.mat = take(nv);
     l.dose_acc = take(sizeof(float) * nv);
     l.sig_t = take(sizeof(float) * G * n_mat);          // stored [G][n_mat]
@@ -127,9 +127,10 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.m2d = take(sizeof(float) * (size_t)n_ang * MP);
     l.d2m = take(sizeof(float) * (size_t)n_ang * MP);
     l.cdd = take(sizeof(float) * per * 4);
-    l.spectrum = take(sizeof(double) * G);
+    l.bm2d = take(sizeof(float) * (size_t)2 * NAP * KP);
+    l.bd2m = take(sizeof(float) * (size_t)2 * NMP * A8);
+    l.signs = take(sizeof(unsigned) * (size_t)8 * MP);
     l.errflag = take(sizeof(int) * 4);
-    l.trace = take(sizeof(long long) * (size_t)(m->nx + DOS_SKEW) * 32 * 4);
     // summed-source mode (dos_uncollided_sum): uncollided moments of all positions and their scalar sum
     l.um = summed ? take(sizeof(float) * G * nv * MP) : 0;
     l.phi_u_sum = summed ? take(sizeof(float) * G * nv) : 0;
@@ -147,33 +148,42 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
     if (xs->n_mat < 1 || xs->n_mat > DOS_MAX_MAT) return fail(nullptr, DOS_ERR_UNSUPPORTED, "n_mat must be 1..16");
     if (xs->n_group < 1 || xs->n_leg < 0 || !xs->sigma_t || !xs->sigma_s || !xs->kerma)
         return fail(nullptr, DOS_ERR_INVALID_ARG, "bad cross-section table");
+    if (xs->n_group > DOS_MAX_G) return fail(nullptr, DOS_ERR_UNSUPPORTED, "more than 64 energy groups");
     if (P_L < 0 || P_L > xs->n_leg) return fail(nullptr, DOS_ERR_SHAPE, "P_L must be 0..n_leg");
     if (P_L > DOS_MAX_L) return fail(nullptr, DOS_ERR_UNSUPPORTED, "P_L > 5");
     if (q->n_ang < 8 || q->n_ang % 8 || !q->mu || !q->eta || !q->xi || !q->w)
         return fail(nullptr, DOS_ERR_INVALID_ARG, "n_ang must be a positive multiple of 8");
-    if (dos_sweep_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_ffma_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 || dos_sweep_v1_angles_per_warp(q->n_ang / 8, P_L) == 0)
-        return fail(nullptr, DOS_ERR_UNSUPPORTED, "angles per octant cannot be split over <= 12 warps of <= 4 angles");
+    if (dos_sweep_ffma_angles_per_warp(q->n_ang / 8, P_L, 0) == 0 && !dos_sweep_umma_supported(q->n_ang / 8, P_L))
+        return fail(nullptr, DOS_ERR_UNSUPPORTED, "no sweep shape for this number of angles per octant");
     return DOS_OK;
 }
 
-// Shape of the sweep CTA (dos_sweep.cu) for the current option values: angle split of an octant over CTAs,
-// angles per compute warp, aux warps, persistent grid.
+// Choice and shape of the sweep for the current option values. The tensor-memory sweep (dos_sweep_umma.cu) is the
+// default wherever the quadrature admits it; the FFMA sweep is the fallback and the A/B partner.
 static cudaError_t configure_sweep(dos_ctx *c)
 {
+    const bool ffma_ok = dos_sweep_ffma_angles_per_warp(c->per_oct, c->L, 0) != 0;
+    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok) || !ffma_ok;
+    if (want_umma) {
+        if (!c->umma_ok) return cudaErrorInvalidValue;
+        int grid = 0;
+        cudaError_t e = dos_sweep_umma_grid(c->L, c->per_oct, c->n_mat, c->n_items_u, &grid);
+        if (e != cudaSuccess) return e;
+        c->grid_u = grid;
+        c->umma = true;
+        return cudaSuccess;
+    }
     int as = c->asplit;
     if (as < 1 || c->per_oct % as) as = 1;
     const int ap = c->per_oct / as;
-    // contractions on the tensor cores from P4 up (28 / 36 moments per cell), FFMA below (measured)
-    const bool mma = c->contraction_pref ? c->contraction_pref == 2 : dos_mpad(c->L) >= 28;
-    const int ag = mma ? dos_sweep_angles_per_warp(ap, c->L, c->ag_pref) : dos_sweep_ffma_angles_per_warp(ap, c->L, c->ag_pref);
+    const int ag = dos_sweep_ffma_angles_per_warp(ap, c->L, c->ag_pref);
     if (ag == 0 || (c->ag_pref > 0 && ag != c->ag_pref)) return cudaErrorInvalidValue;
-    const int nx = mma ? dos_sweep_aux_warps(ap, c->L, ag, c->aux_pref) : dos_sweep_ffma_aux_warps(ap, c->L, ag, c->aux_pref);
-    if (ap / ag + nx + 2 > (mma ? 20 : 24)) return cudaErrorInvalidValue;
+    const int nx = dos_sweep_ffma_aux_warps(ap, c->L, ag, c->aux_pref);
+    if (ap / ag + nx + 2 > 24) return cudaErrorInvalidValue;
     int grid = 0;
-    cudaError_t e = mma ? dos_sweep_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, &grid)
-                        : dos_sweep_ffma_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, &grid);
+    cudaError_t e = dos_sweep_ffma_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, c->two_per_sm, &grid);
     if (e != cudaSuccess) return e;
-    c->asplit = as; c->ag = ag; c->n_grp = ap / ag; c->n_aux = nx; c->grid = grid; c->mma = mma;
+    c->asplit = as; c->ag = ag; c->n_grp = ap / ag; c->n_aux = nx; c->grid = grid; c->umma = false;
     return cudaSuccess;
 }
 
@@ -243,16 +253,16 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->ntj = (mesh->ny + DOS_TJ - 1) / DOS_TJ;
     c->ntk = (mesh->nz + DOS_TK - 1) / DOS_TK;
     c->n_items = 8 * c->ntj * c->ntk;
-    c->impl = 0;
-    c->trace_item = -1;
+    c->n_items_u = 2 * c->ntj * c->ntk;
     c->can_sum = can_sum; c->summed = false;
     c->contraction_pref = 0;
     c->ag_pref = c->aux_pref = 0;
     c->asplit = default_asplit(per, c->n_items);
     c->chunk = 4;
-    c->ag1 = dos_sweep_v1_angles_per_warp(per, L);
-    c->n_grp1 = per / c->ag1;
-    c->chunk1 = mesh->nx <= 64 ? 8 : 16;
+    c->two_per_sm = 1;
+    c->umma = false;
+    c->grid = c->grid_u = 0;
+    c->mat_checked = false;
     c->nv = (size_t)mesh->nx * mesh->ny * mesh->nz;
     c->stream = (cudaStream_t)cuda_stream;
     c->d_mat = d_material_ids;
@@ -295,15 +305,54 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
         cdd[t * 4 + 0] = (float)cx; cdd[t * 4 + 1] = (float)cy; cdd[t * 4 + 2] = (float)cz;
         cdd[t * 4 + 3] = (float)(cx + cy + cz);
     }
-    // work items, tile-diagonal major: every item's upwind tiles (tj-1,tk), (tj,tk-1) come earlier
-    std::vector<int> items;
+    // work items, tile-diagonal major: every item's upwind tiles (tj-1,tk), (tj,tk-1) come earlier.
+    // FFMA sweep: (octant, tile); tensor-memory sweep: (octant quad, tile)
+    std::vector<int> items, items_u;
     items.reserve(c->n_items);
+    items_u.reserve(c->n_items_u);
     for (int d = 0; d <= c->ntj + c->ntk - 2; ++d)
         for (int tj = 0; tj < c->ntj; ++tj) {
             const int tk = d - tj;
             if (tk < 0 || tk >= c->ntk) continue;
             for (int o = 0; o < 8; ++o) items.push_back(o | (tj << 3) | (tk << 17));
+            for (int qd = 0; qd < 2; ++qd) items_u.push_back(qd | (tj << 3) | (tk << 17));
         }
+    // Tensor-memory sweep tables. Y_lm of a direction mirrored into octant o is +-Y_lm of the octant-0 direction, the
+    // sign depending on (l, m) and the mirror only: signs[o][lm]. The UMMA B operands hold octant 0's coefficients,
+    // split into TF32 hi + lo, in the no-swizzle K-major core-matrix layout (8 rows x 16 bytes).
+    const int KP = (MP + 7) & ~7, NCH = KP / 4, A8 = (per + 7) & ~7, NAP = (per + 15) & ~15, NMP = (MP + 15) & ~15;
+    std::vector<unsigned> signs((size_t)8 * MP, 0u);
+    std::vector<float> bm2d((size_t)2 * NAP * KP, 0.f), bd2m((size_t)2 * NMP * A8, 0.f);
+    bool umma_ok = dos_sweep_umma_supported(per, L) != 0;
+    for (int o = 0; o < 8 && umma_ok; ++o)
+        for (int lm = 0; lm < M; ++lm) {
+            int tbest = 0;
+            for (int t = 1; t < per; ++t)
+                if (std::fabs(m2d[(size_t)t * MP + lm]) > std::fabs(m2d[(size_t)tbest * MP + lm])) tbest = t;
+            const bool neg = (m2d[((size_t)o * per + tbest) * MP + lm] < 0.f) != (m2d[(size_t)tbest * MP + lm] < 0.f);
+            signs[(size_t)o * MP + lm] = neg ? 0x80000000u : 0u;
+            for (int t = 0; t < per; ++t) {       // the mirror relation must hold exactly, for both tables
+                const float sg = neg ? -1.f : 1.f;
+                if (m2d[((size_t)o * per + t) * MP + lm] != sg * m2d[(size_t)t * MP + lm] ||
+                    d2m[((size_t)o * per + t) * MP + lm] != sg * d2m[(size_t)t * MP + lm]) umma_ok = false;
+            }
+        }
+    auto tf32 = [](float x) {
+        unsigned b; std::memcpy(&b, &x, 4);
+        b = (b + 0x1000u) & 0xffffe000u;
+        float r; std::memcpy(&r, &b, 4);
+        return r;
+    };
+    for (int n = 0; n < per; ++n)
+        for (int k = 0; k < MP; ++k) {
+            const size_t im = ((size_t)(n / 8) * NCH + k / 4) * 32 + (n % 8) * 4 + (k % 4);              // (angle n, moment k)
+            const float vm = m2d[(size_t)n * MP + k], hm = tf32(vm);
+            bm2d[im] = hm; bm2d[(size_t)NAP * KP + im] = tf32(vm - hm);
+            const size_t id = ((size_t)(k / 8) * (A8 / 4) + n / 4) * 32 + (k % 8) * 4 + (n % 4);         // (moment k, angle n)
+            const float vd = d2m[(size_t)n * MP + k], hd = tf32(vd);
+            bd2m[id] = hd; bd2m[(size_t)NMP * A8 + id] = tf32(vd - hd);
+        }
+    c->umma_ok = umma_ok;
 
     auto up = [&](size_t off, const void *src, size_t bytes) {
         return cudaMemcpyAsync(c->ws + off, src, bytes, cudaMemcpyHostToDevice, c->stream);
@@ -316,10 +365,15 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     if (e == cudaSuccess) e = up(lay.d2m, d2m.data(), sizeof(float) * d2m.size());
     if (e == cudaSuccess) e = up(lay.cdd, cdd.data(), sizeof(float) * cdd.size());
     if (e == cudaSuccess) e = up(lay.items, items.data(), sizeof(int) * items.size());
+    if (e == cudaSuccess) e = up(lay.items_u, items_u.data(), sizeof(int) * items_u.size());
+    if (e == cudaSuccess) e = up(lay.bm2d, bm2d.data(), sizeof(float) * bm2d.size());
+    if (e == cudaSuccess) e = up(lay.bd2m, bd2m.data(), sizeof(float) * bd2m.size());
+    if (e == cudaSuccess) e = up(lay.signs, signs.data(), sizeof(unsigned) * signs.size());
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.errflag, 0, sizeof(int) * 4, c->stream);
+    // the whole grid is checked once, here (dos.h: ids < n_mat); every kernel also clamps the id it indexes with
+    if (e == cudaSuccess) e = dos_launch_validate_material(c->nv, c->d_mat, n_mat, (int *)(c->ws + lay.errflag), c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // host vectors go out of scope
     if (e == cudaSuccess) e = configure_sweep(c);
-    if (e == cudaSuccess) e = dos_sweep_v1_grid(L, c->ag1, per, n_mat, c->n_items, &c->grid1);
     if (e != cudaSuccess) {
         std::string msg = std::string("dos_create: ") + cudaGetErrorString(e);
         delete c;
@@ -386,8 +440,14 @@ static void prof_collect(dos_ctx *c)
 extern "C" dos_status dos_set_material_host(dos_ctx *c, const uint8_t *h_material_ids)
 {
     if (!c || !h_material_ids) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    // The copy is enqueued; with pageable memory the runtime stages it before returning, with pinned memory the
+    // caller's buffer must stay untouched until the stream reaches this point (dos.h).
     CUDA_TRY(c, cudaMemcpyAsync(c->ws + c->lay.mat, h_material_ids, c->nv, cudaMemcpyHostToDevice, c->stream));
     c->d_mat = (const uint8_t *)(c->ws + c->lay.mat);
+    // a new grid: the "bad material id" flag starts afresh and the grid is checked again
+    CUDA_TRY(c, cudaMemsetAsync(c->ws + c->lay.errflag, 0, sizeof(int), c->stream));
+    CUDA_TRY(c, dos_launch_validate_material(c->nv, c->d_mat, c->n_mat, (int *)(c->ws + c->lay.errflag), c->stream));
+    c->launches += 1;
     c->state = 0;
     return DOS_OK;
 }
@@ -418,18 +478,17 @@ static dos_status uncollided_impl(dos_ctx *c, const dos_source *source, const fl
                 return fail(c, DOS_ERR_INVALID_ARG, "source coincides with a voxel centre");
         }
     }
-    std::vector<double> sp(c->G);
+    SpectrumDev sp;                                  // travels in the kernel's parameters: nothing to copy, nothing to wait for
+    for (int g = 0; g < DOS_MAX_G; ++g) sp.s[g] = 0.0;
     for (int g = 0; g < c->G; ++g) {
         if (!(spectrum[g] >= 0.f)) return fail(c, DOS_ERR_INVALID_ARG, "spectrum must be >= 0");
-        sp[g] = (double)spectrum[g];
+        sp.s[g] = (double)spectrum[g];
     }
     c->src = *source;
-    CUDA_TRY(c, cudaMemcpyAsync(c->ws + c->lay.spectrum, sp.data(), sizeof(double) * c->G, cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));   // sp is a stack-lifetime buffer
     float *phi_u = (float *)(c->ws + c->lay.phi_u);
     prof_begin(c, 1);
     CUDA_TRY(c, dos_launch_raytrace(mesh_dev(c->mesh), source_dev(*source), c->d_mat, c->n_mat, c->G,
-                                    (const float *)(c->ws + c->lay.sig_t), (const double *)(c->ws + c->lay.spectrum),
+                                    (const float *)(c->ws + c->lay.sig_t), sp,
                                     phi_u, (int *)(c->ws + c->lay.errflag), c->stream));
     prof_end(c);
     c->launches += 1;
@@ -456,6 +515,15 @@ extern "C" dos_status dos_uncollided_sum(dos_ctx *c, const dos_source *source, c
     return uncollided_impl(c, source, spectrum, d_phi_u_out, first ? 1 : 2);
 }
 
+extern "C" dos_status dos_uncollided_total(dos_ctx *c, float *d_phi_u_out)
+{
+    if (!c || !d_phi_u_out) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    if (c->state < 1) return fail(c, DOS_ERR_STATE, "dos_uncollided_total before dos_uncollided");
+    const float *src = (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u));
+    CUDA_TRY(c, cudaMemcpyAsync(d_phi_u_out, src, sizeof(float) * c->G * c->nv, cudaMemcpyDeviceToDevice, c->stream));
+    return DOS_OK;
+}
+
 extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
 {
     if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
@@ -468,41 +536,37 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
     int *done = (int *)(c->ws + c->lay.done), *queue = (int *)(c->ws + c->lay.queue);
     const MeshDev md = mesh_dev(c->mesh);
     const SourceDev sd = source_dev(c->src);
-    SweepArgs a1;                       // first version (option sweep_impl = 1)
-    a1.nx = c->mesh.nx; a1.ny = c->mesh.ny; a1.nz = c->mesh.nz;
-    a1.ntj = c->ntj; a1.ntk = c->ntk; a1.n_items = c->n_items; a1.per_oct = c->per_oct; a1.n_grp = c->n_grp1;
-    a1.chunk = c->chunk1; a1.n_mat = c->n_mat;
-    a1.items = (const int *)(c->ws + c->lay.items);
-    a1.Q = q; a1.mat = c->d_mat;
-    a1.m2d = (const float *)(c->ws + c->lay.m2d); a1.d2m = (const float *)(c->ws + c->lay.d2m);
-    a1.cdd = (const float *)(c->ws + c->lay.cdd);
-    a1.fy = (float *)(c->ws + c->lay.fy); a1.fz = (float *)(c->ws + c->lay.fz);
-    a1.done = done; a1.queue = queue;
-    a1.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
-    Sweep2Args a;
-    a.nx = a1.nx; a.ny = a1.ny; a.nz = a1.nz; a.ntj = a1.ntj; a.ntk = a1.ntk; a.n_items = a1.n_items;
+    Sweep2Args a;                       // FFMA sweep
+    a.nx = c->mesh.nx; a.ny = c->mesh.ny; a.nz = c->mesh.nz; a.ntj = c->ntj; a.ntk = c->ntk;
     a.per_oct = c->per_oct / c->asplit; a.per_oct_full = c->per_oct; a.a_split = c->asplit;
-    a.n_items = c->n_items * c->asplit; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = a1.n_mat;
-    a.items = a1.items; a.Q = q; a.mat = c->d_mat; a.m2d = a1.m2d; a.d2m = a1.d2m; a.cdd = a1.cdd;
-    a.fy = a1.fy; a.fz = a1.fz; a.done = done; a.queue = queue; a.abort_flag = a1.abort_flag;
-    a.trace = c->trace_item >= 0 ? (long long *)(c->ws + c->lay.trace) : nullptr;
-    a.trace_item = c->trace_item;
-    const int n_flags = c->impl == 1 ? c->n_items * c->n_grp1 : c->n_items * c->asplit;
+    a.n_items = c->n_items * c->asplit; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = c->n_mat;
+    a.items = (const int *)(c->ws + c->lay.items); a.Q = q; a.mat = c->d_mat;
+    a.m2d = (const float *)(c->ws + c->lay.m2d); a.d2m = (const float *)(c->ws + c->lay.d2m);
+    a.cdd = (const float *)(c->ws + c->lay.cdd);
+    a.fy = (float *)(c->ws + c->lay.fy); a.fz = (float *)(c->ws + c->lay.fz); a.done = done; a.queue = queue;
+    a.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
+    SweepUArgs u;                       // tensor-memory sweep
+    u.nx = a.nx; u.ny = a.ny; u.nz = a.nz; u.ntj = a.ntj; u.ntk = a.ntk; u.n_items = c->n_items_u; u.per_oct = c->per_oct;
+    u.MP = c->MP; u.chunk = c->chunk; u.n_mat = c->n_mat;
+    u.items = (const int *)(c->ws + c->lay.items_u); u.Q = q; u.mat = c->d_mat; u.cdd = a.cdd;
+    u.bm2d = (const float *)(c->ws + c->lay.bm2d); u.bd2m = (const float *)(c->ws + c->lay.bd2m);
+    u.signs = (const unsigned *)(c->ws + c->lay.signs);
+    u.fy = a.fy; u.fz = a.fz; u.done = done; u.queue = queue; u.abort_flag = a.abort_flag;
+    const int n_flags = c->umma ? c->n_items_u : c->n_items * c->asplit;
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
-        CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
+        CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
                                             c->summed ? (const float *)(c->ws + c->lay.um) : nullptr,
                                             phi_all, qfix, c->stream));
         c->launches += 1;
-        a.phi = a1.phi = phi;
-        a.sig_t = a1.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
+        a.phi = u.phi = phi;
+        a.sig_t = u.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
         for (int it = 0; it < n_iter; ++it) {
-            CUDA_TRY(c, dos_launch_source_update(c->nv, c->d_mat, c->G, c->n_leg, c->L, g, sig_s, qfix, phi, q, it == 0,
+            CUDA_TRY(c, dos_launch_source_update(c->nv, c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, sig_s, qfix, phi, q, it == 0,
                                                  done, n_flags, queue, c->stream));
             prof_begin(c, 0);
-            if (c->impl == 1) CUDA_TRY(c, dos_launch_sweep_v1(a1, c->L, c->ag1, c->grid1, c->stream));
-            else if (c->mma) CUDA_TRY(c, dos_launch_sweep(a, c->L, c->ag, c->grid, c->stream));
-            else CUDA_TRY(c, dos_launch_sweep_ffma(a, c->L, c->ag, c->grid, c->stream));
+            if (c->umma) CUDA_TRY(c, dos_launch_sweep_umma(u, c->L, c->grid_u, c->stream));
+            else CUDA_TRY(c, dos_launch_sweep_ffma(a, c->L, c->ag, c->grid, c->two_per_sm, c->stream));
             prof_end(c);
             c->launches += 2;
         }
@@ -562,57 +626,41 @@ extern "C" dos_status dos_dose_host(dos_ctx *c, float *h_dose, int32_t accumulat
 extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value)
 {
     if (!c || !name) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    // sweep-shape options: set, re-configure, and on failure restore what was in force
+    const int old_ag = c->ag_pref, old_aux = c->aux_pref, old_as = c->asplit, old_pref = c->contraction_pref, old_two = c->two_per_sm;
+    bool reshape = false;
     if (!strcmp(name, "sweep_chunk")) {
         if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_chunk must be >= 1");
-        c->chunk = c->chunk1 = (int)value;
-    } else if (!strcmp(name, "sweep_impl")) {
-        if (value != 0 && value != 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_impl must be 0 or 1");
-        c->impl = (int)value;
-    } else if (!strcmp(name, "sweep_angles_per_warp") || !strcmp(name, "sweep_aux_warps") || !strcmp(name, "sweep_angle_split")) {
-        // 0 = library default
-        const int old_ag = c->ag_pref, old_aux = c->aux_pref, old_as = c->asplit;
-        if (value < 0 || value > 16) return fail(c, DOS_ERR_INVALID_ARG, std::string(name) + " out of range");
-        if (name[6] == 'a' && name[8] == 'g' && name[11] == '_' && name[12] == 's') {     // sweep_angle_split
-            if (value > 8 || (value > 0 && c->per_oct % value)) return fail(c, DOS_ERR_INVALID_ARG, "sweep_angle_split must divide the angles per octant (<= 8)");
-            c->asplit = value > 0 ? (int)value : default_asplit(c->per_oct, c->n_items);
-        } else if (name[7] == 'n') {
-            c->ag_pref = (int)value;
-        } else {
-            c->aux_pref = (int)value;
-        }
-        cudaError_t e = configure_sweep(c);
-        if (e != cudaSuccess) {
-            c->ag_pref = old_ag; c->aux_pref = old_aux; c->asplit = old_as;
-            configure_sweep(c);
-            return fail(c, DOS_ERR_INVALID_ARG, std::string(name) + ": not admissible for this quadrature");
-        }
-    } else if (!strcmp(name, "sweep_trace_item")) {
-        if (value < -1 || value >= c->n_items * c->asplit) return fail(c, DOS_ERR_INVALID_ARG, "sweep_trace_item out of range");
-        if (value >= 0 && !dos_sweep_trace_compiled())
-            return fail(c, DOS_ERR_UNSUPPORTED, "sweep_trace_item: libdos was built without -DDOS_SWEEP_TRACE=1");
-        c->trace_item = (int)value;
-        CUDA_TRY(c, cudaMemsetAsync(c->ws + c->lay.trace, 0, sizeof(long long) * (size_t)(c->mesh.nx + DOS_SKEW) * 128, c->stream));
+        c->chunk = (int)value;
+    } else if (!strcmp(name, "sweep_angles_per_warp")) {
+        if (value < 0 || value > 16) return fail(c, DOS_ERR_INVALID_ARG, "sweep_angles_per_warp out of range");
+        c->ag_pref = (int)value; reshape = true;
+    } else if (!strcmp(name, "sweep_aux_warps")) {
+        if (value < 0 || value > 16) return fail(c, DOS_ERR_INVALID_ARG, "sweep_aux_warps out of range");
+        c->aux_pref = (int)value; reshape = true;
+    } else if (!strcmp(name, "sweep_angle_split")) {
+        if (value < 0 || value > 8 || (value > 0 && c->per_oct % value))
+            return fail(c, DOS_ERR_INVALID_ARG, "sweep_angle_split must divide the angles per octant (<= 8)");
+        c->asplit = value > 0 ? (int)value : default_asplit(c->per_oct, c->n_items); reshape = true;
     } else if (!strcmp(name, "sweep_contraction")) {
-        if (value < 0 || value > 2) return fail(c, DOS_ERR_INVALID_ARG, "sweep_contraction must be 0 (auto), 1 (FFMA) or 2 (tensor cores)");
-        const int old = c->contraction_pref;
-        c->contraction_pref = (int)value;
-        if (configure_sweep(c) != cudaSuccess) {
-            c->contraction_pref = old;
-            configure_sweep(c);
-            return fail(c, DOS_ERR_INVALID_ARG, "sweep_contraction: not admissible with the current sweep shape options");
-        }
+        if (value < 0 || value > 2) return fail(c, DOS_ERR_INVALID_ARG, "sweep_contraction must be 0 (auto), 1 (FFMA) or 2 (tensor memory)");
+        c->contraction_pref = (int)value; reshape = true;
     } else if (!strcmp(name, "sweep_two_per_sm")) {
-        dos_sweep_set_two_per_sm(value & 1);       // bit 0: tensor-core sweep, bit 1: FFMA sweep
-        dos_sweep_ffma_set_two_per_sm((value & 4) ? 2 : ((value & 2) ? 1 : 0));   // bit 2: also for few items per SM
-        CUDA_TRY(c, configure_sweep(c));
+        if (value < 0 || value > 2) return fail(c, DOS_ERR_INVALID_ARG, "sweep_two_per_sm must be 0, 1 or 2");
+        c->two_per_sm = (int)value; reshape = true;
     } else if (!strcmp(name, "profile")) {
         c->profile = value != 0;
     } else if (!strcmp(name, "sweep_grid")) {
         if (value < 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_grid must be >= 1");
-        c->grid1 = (int)(value < c->n_items ? value : c->n_items);
         c->grid = (int)(value < c->n_items * c->asplit ? value : c->n_items * c->asplit);
+        c->grid_u = (int)(value < c->n_items_u ? value : c->n_items_u);
     } else {
         return fail(c, DOS_ERR_INVALID_ARG, std::string("unknown option ") + name);
+    }
+    if (reshape && configure_sweep(c) != cudaSuccess) {
+        c->ag_pref = old_ag; c->aux_pref = old_aux; c->asplit = old_as; c->contraction_pref = old_pref; c->two_per_sm = old_two;
+        configure_sweep(c);
+        return fail(c, DOS_ERR_INVALID_ARG, std::string(name) + ": not admissible for this quadrature / sweep shape");
     }
     return DOS_OK;
 }
@@ -625,16 +673,6 @@ extern "C" dos_status dos_profile(dos_ctx *c, dos_profile_t *out)
     out->sweep_ms = c->acc_ms[0]; out->sweep_launches = c->acc_n[0];
     out->raytrace_ms = c->acc_ms[1]; out->raytrace_launches = c->acc_n[1];
     out->kernel_launches = c->launches;
-    return DOS_OK;
-}
-
-extern "C" dos_status dos_sweep_trace_host(dos_ctx *c, int64_t *h_trace, size_t n)
-{
-    if (!c || !h_trace) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
-    const size_t have = (size_t)(c->mesh.nx + DOS_SKEW) * 128;
-    if (n > have) n = have;
-    CUDA_TRY(c, cudaMemcpyAsync(h_trace, c->ws + c->lay.trace, sizeof(int64_t) * n, cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return DOS_OK;
 }
 

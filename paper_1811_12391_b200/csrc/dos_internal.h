@@ -14,36 +14,7 @@
 // number of moments (L+1)^2 padded to a multiple of 4 so that a cell's moments are whole float4s
 static inline __host__ __device__ int dos_mpad(int L) { return (((L + 1) * (L + 1)) + 3) & ~3; }
 
-// Arguments of one sweep launch (all 8 octants, one energy group, one source iteration).
-struct SweepArgs {
-    int nx, ny, nz;
-    int ntj, ntk;            // tiles along j and k
-    int n_items;             // 8 * ntj * ntk work items (octant, tile)
-    int per_oct;             // angles per octant (A)
-    int n_grp;               // angle groups = warps per CTA (A / AG)
-    int chunk;               // cells along x between flag publications
-    int n_mat;
-    const int *items;        // [n_items] packed (octant | tj << 3 | tk << 17), dependency-safe order
-    const float *Q;          // [Nv][MP] frozen source moments
-    float *phi;              // [Nv][MP] accumulates w Y psi (zeroed before the launch)
-    const uint8_t *mat;      // [Nv]
-    const float *sig_t;      // [n_mat] total cross section of this group
-    const float *m2d;        // [8][A][MP] (2l+1) Y_lm(Omega_n)
-    const float *d2m;        // [8][A][MP] w_n Y_lm(Omega_n)
-    const float *cdd;        // [A][4] cx, cy, cz, cx+cy+cz  (2|Omega_d|/Delta_d; same for all octants)
-    float *fy;               // [8][A][ntj][nz'][nx'] y-face fluxes leaving tile row tj (oriented indices)
-    float *fz;               // [8][A][ntk][ny'][nx'] z-face fluxes leaving tile row tk
-    int *done;               // [n_items (by id)][n_grp] cells along x finished and published
-    int *queue;              // work-queue head
-    int *abort_flag;         // set by the watchdog; every waiting warp then stops waiting
-};
-
-// dos_sweep_v1.cu (first version; option sweep_impl=1)
-cudaError_t dos_launch_sweep_v1(const SweepArgs &a, int L, int ang_per_warp, int grid, cudaStream_t s);
-int dos_sweep_v1_angles_per_warp(int per_oct, int L);
-cudaError_t dos_sweep_v1_grid(int L, int ang_per_warp, int per_oct, int n_mat, int n_items, int *grid_out);
-
-// ---- dos_sweep.cu: the sweep the library uses by default ----
+// ---- dos_sweep_ffma.cu: the sweep with FFMA contractions ----
 #define DOS_FACE_PAD 8      // diagonal index d = x + (lane offset) runs over [0, nx + DOS_FACE_PAD)
 #define DOS_PREFETCH_Q 6    // steps between issuing the cp.async of a step's source moments and using them
 #define DOS_RING_Q 8
@@ -80,19 +51,38 @@ struct Sweep2Args {
     int *done;               // [n_items (by id)] steps finished and published
     int *queue;              // work-queue head
     int *abort_flag;         // set by the watchdog; every waiting CTA then stops waiting
-    long long *trace;        // optional [nx + DOS_SKEW][32][4] SM-clock timeline of item `trace_item` (or null)
-    int trace_item;
 };
 
-cudaError_t dos_launch_sweep(const Sweep2Args &a, int L, int ang_per_warp, int grid, cudaStream_t s);
-int dos_sweep_angles_per_warp(int per_oct, int L, int prefer);
-cudaError_t dos_sweep_grid(int L, int ang_per_warp, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out);
-int dos_sweep_aux_warps(int per_oct, int L, int ang_per_warp, int prefer);
-// dos_sweep_ffma.cu: the same sweep with FFMA contractions (few moments per cell)
-cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ang_per_warp, int grid, cudaStream_t s);
+cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ang_per_warp, int grid, int two_per_sm, cudaStream_t s);
 int dos_sweep_ffma_angles_per_warp(int per_oct, int L, int prefer);
-cudaError_t dos_sweep_ffma_grid(int L, int ang_per_warp, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out);
+cudaError_t dos_sweep_ffma_grid(int L, int ang_per_warp, int n_aux, int per_oct, int n_mat, int n_items, int two_per_sm, int *grid_out);
 int dos_sweep_ffma_aux_warps(int per_oct, int L, int ang_per_warp, int prefer);
-void dos_sweep_ffma_set_two_per_sm(int on);
-void dos_sweep_set_two_per_sm(int on);   // allow the 64-register, 2-CTAs-per-SM variant (process-wide)
-int dos_sweep_trace_compiled();   // 1 if dos_sweep.cu was built with -DDOS_SWEEP_TRACE=1
+
+// ---- dos_sweep_umma.cu: the sweep on the tensor-memory path (tcgen05.mma + bulk copies + mbarrier rings) ----
+// One launch = all 8 octants, one energy group, one source iteration. Work item = (octant quad, tile).
+struct SweepUArgs {
+    int nx, ny, nz;
+    int ntj, ntk;            // tiles along j and k
+    int n_items;             // 2 * ntj * ntk work items (quad, tile)
+    int per_oct;             // angles per octant (A)
+    int MP;                  // moments per cell, padded to a multiple of 4
+    int chunk;               // steps between flag publications
+    int n_mat;
+    const int *items;        // [n_items] packed (quad | tj << 3 | tk << 17), dependency-safe order
+    const float *Q;          // [Nv][MP] frozen source moments
+    float *phi;              // [Nv][MP] accumulates w Y psi (zeroed before the launch)
+    const uint8_t *mat;      // [Nv]
+    const float *sig_t;      // [n_mat] total cross section of this group
+    const float *cdd;        // [A][4] cx, cy, cz, cx+cy+cz
+    const float *bm2d;       // UMMA B operand of the moment-to-discrete: [hi, lo][NAP/8][KP/4][8][4], (angle, lm) = (2l+1) Y_lm, octant 0
+    const float *bd2m;       // UMMA B operand of the discrete-to-moment: [hi, lo][NMP/8][A8/4][8][4], (lm, angle) = w Y_lm, octant 0
+    const unsigned *signs;   // [8][MP] sign bit of Y_lm(mirror_o Omega) / Y_lm(Omega)
+    float *fy;               // [8 * ntj * ntk (by octant, tile)][nx + PAD][A][TK] y-face fluxes leaving a tile, by diagonal
+    float *fz;               // [8 * ntj * ntk][nx + PAD][A][TJ]
+    int *done;               // [2 * ntj * ntk (by quad, tile)] steps finished and published
+    int *queue;              // work-queue head
+    int *abort_flag;
+};
+int dos_sweep_umma_supported(int per_oct, int L);
+cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int *grid_out);
+cudaError_t dos_launch_sweep_umma(const SweepUArgs &a, int L, int grid, cudaStream_t s);

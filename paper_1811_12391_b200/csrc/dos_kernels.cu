@@ -12,13 +12,13 @@ constexpr int RT_THREADS = 128;
 // a1. Uncollided fluence ("computable with a ray-tracing algorithm"; R6-R9).
 // One thread per voxel. The ray is walked BACKWARDS, from the voxel centre towards the source, with
 // exact plane-crossing parameters (Siddon): beta in [0,1] along c -> s; the next crossing on each axis
-// is recomputed from its plane index (no accumulated increments). Runs of equal material are merged:
+// advances by a per-axis constant in fp64 (<= 1e-13 drift over a few hundred steps). Runs of equal material are merged:
 // the length of a run is (beta_end - beta_start) r, added to that material's slot; the n_mat x G
 // contraction with sigma_t and the exponential happen once per voxel, all in fp64.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(RT_THREADS) raytrace_kernel(MeshDev m, SourceDev s, const uint8_t *__restrict__ mat,
                                                               int n_mat, int G, const float *__restrict__ sig_t_gm,
-                                                              const double *__restrict__ spectrum,
+                                                              const SpectrumDev spectrum,
                                                               float *__restrict__ phi_u, int *errflag)
 {
     __shared__ double s_len[DOS_MAX_MAT][RT_THREADS];
@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(RT_THREADS) raytrace_kernel(MeshDev m, SourceD
     for (int g = 0; g < G; ++g) {
         double tau = 0.0;
         for (int t = 0; t < n_mat; ++t) tau += (double)sig_t_gm[g * n_mat + t] * s_len[t][threadIdx.x];
-        const float v = inside ? (float)(spectrum[g] * exp(-tau) * geo) : 0.f;      // outside the beam: exactly 0 (R16)
+        const float v = inside ? (float)(spectrum.s[g] * exp(-tau) * geo) : 0.f;      // outside the beam: exactly 0 (R16)
         if (in_mesh) phi_u[(size_t)g * nv + cell] = v;
     }
 }
@@ -126,7 +126,7 @@ __device__ __forceinline__ void dev_ylm(double mu, double eta, double xi, float 
 }  // namespace
 
 cudaError_t dos_launch_raytrace(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int n_mat, int G,
-                                const float *sig_t_gm, const double *spectrum, float *phi_u, int *errflag,
+                                const float *sig_t_gm, const SpectrumDev &spectrum, float *phi_u, int *errflag,
                                 cudaStream_t st)
 {
     const size_t nv = (size_t)m.nx * m.ny * m.nz;
@@ -144,7 +144,7 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 template <int L>
 __global__ void __launch_bounds__(128) group_source_kernel(MeshDev m, SourceDev s, const uint8_t *__restrict__ mat,
-                                                           int G, int n_leg, int g, int g_lo,
+                                                           int n_mat, int G, int n_leg, int g, int g_lo,
                                                            const float *__restrict__ sig_s,
                                                            const float *__restrict__ phi_u,
                                                            const float *__restrict__ um,
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(128) group_source_kernel(MeshDev m, SourceDev 
     const size_t nv = (size_t)m.nx * m.ny * m.nz;
     const size_t cell = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (cell >= nv) return;
-    const int mt = mat[cell];
+    const int mt = min((int)mat[cell], n_mat - 1);       // ids are validated once per grid (validate_material_kernel); never index past a table
     const float *ss = sig_s + (size_t)mt * (n_leg + 1) * G * G;     // [l][from][to]
     float acc[MP];
 #pragma unroll
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(128) group_source_kernel(MeshDev m, SourceDev 
 // hand-off flags and work-queue head.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) source_update_kernel(size_t nv, int MV, int M, const uint8_t *__restrict__ mat,
-                                                            int G, int n_leg, int g, const float *__restrict__ sig_s,
+                                                            int n_mat, int G, int n_leg, int g, const float *__restrict__ sig_s,
                                                             const float4 *__restrict__ qfix, float4 *__restrict__ phi,
                                                             float4 *__restrict__ q, int first, int *done, int n_flags,
                                                             int *queue)
@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(256) source_update_kernel(size_t nv, int MV, i
     const int v = (int)(t - cell * MV);
     float4 out = qfix[t];
     if (!first) {
-        const float *ss = sig_s + (size_t)mat[cell] * (n_leg + 1) * G * G + (size_t)g * G + g;   // + l*G*G
+        const float *ss = sig_s + (size_t)min((int)mat[cell], n_mat - 1) * (n_leg + 1) * G * G + (size_t)g * G + g;   // + l*G*G
         const float4 p = phi[t];
         const float pv[4] = {p.x, p.y, p.z, p.w};
         float ov[4] = {out.x, out.y, out.z, out.w};
@@ -261,13 +261,13 @@ __global__ void fluence_kernel(size_t nv, int G, int MP, const float *__restrict
 }
 
 // a8. D(c) = sum_g K[m(c)][g] (phi_u^g + phi_c^g)(c); groups summed in index order
-__global__ void dose_kernel(size_t nv, const uint8_t *__restrict__ mat, int G, int MP, const float *__restrict__ kerma,
+__global__ void dose_kernel(size_t nv, const uint8_t *__restrict__ mat, int n_mat, int G, int MP, const float *__restrict__ kerma,
                             const float *__restrict__ phi_u, const float *__restrict__ phi_all, float *dose,
                             int accumulate)
 {
     const size_t cell = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (cell >= nv) return;
-    const float *kr = kerma + (size_t)mat[cell] * G;
+    const float *kr = kerma + (size_t)min((int)mat[cell], n_mat - 1) * G;
     float d = 0.f;
     for (int g = 0; g < G; ++g) d = fmaf(kr[g], phi_u[(size_t)g * nv + cell] + phi_all[((size_t)g * nv + cell) * MP], d);
     dose[cell] = accumulate ? dose[cell] + d : d;
@@ -275,25 +275,25 @@ __global__ void dose_kernel(size_t nv, const uint8_t *__restrict__ mat, int G, i
 
 }  // namespace
 
-cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int G, int n_leg, int L,
+cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int n_mat, int G, int n_leg, int L,
                                     int g, int g_lo, const float *sig_s, const float *phi_u, const float *um,
                                     const float *phi_all, float *qfix, cudaStream_t st)
 {
     const size_t nv = (size_t)m.nx * m.ny * m.nz;
     const unsigned grid = (unsigned)((nv + 127) / 128);
     switch (L) {
-        case 0: group_source_kernel<0><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
-        case 1: group_source_kernel<1><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
-        case 2: group_source_kernel<2><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
-        case 3: group_source_kernel<3><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
-        case 4: group_source_kernel<4><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
-        case 5: group_source_kernel<5><<<grid, 128, 0, st>>>(m, s, mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 0: group_source_kernel<0><<<grid, 128, 0, st>>>(m, s, mat, n_mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 1: group_source_kernel<1><<<grid, 128, 0, st>>>(m, s, mat, n_mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 2: group_source_kernel<2><<<grid, 128, 0, st>>>(m, s, mat, n_mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 3: group_source_kernel<3><<<grid, 128, 0, st>>>(m, s, mat, n_mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 4: group_source_kernel<4><<<grid, 128, 0, st>>>(m, s, mat, n_mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
+        case 5: group_source_kernel<5><<<grid, 128, 0, st>>>(m, s, mat, n_mat, G, n_leg, g, g_lo, sig_s, phi_u, um, phi_all, qfix); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
 }
 
-cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int G, int n_leg, int L, int g, const float *sig_s,
+cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int n_mat, int G, int n_leg, int L, int g, const float *sig_s,
                                      const float *qfix, float *phi, float *q, int first, int *done, int n_flags,
                                      int *queue, cudaStream_t st)
 {
@@ -301,7 +301,7 @@ cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int G, int n
     size_t n = nv * MV;
     if ((size_t)n_flags > n) n = (size_t)n_flags;
     const unsigned grid = (unsigned)((n + 255) / 256);
-    source_update_kernel<<<grid, 256, 0, st>>>(nv, MV, M, mat, G, n_leg, g, sig_s, (const float4 *)qfix, (float4 *)phi,
+    source_update_kernel<<<grid, 256, 0, st>>>(nv, MV, M, mat, n_mat, G, n_leg, g, sig_s, (const float4 *)qfix, (float4 *)phi,
                                                (float4 *)q, first, done, n_flags, queue);
     return cudaGetLastError();
 }
@@ -374,6 +374,34 @@ cudaError_t dos_launch_um_accumulate(const MeshDev &m, const SourceDev &s, int G
     return cudaGetLastError();
 }
 
+// Whole-grid check of the material ids (dos.h: "values < n_mat"), run once per grid: errflag[0] = 1 if any id >= n_mat.
+namespace {
+__global__ void validate_material_kernel(size_t nv, const uint8_t *__restrict__ mat, int n_mat, int *errflag)
+{
+    const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 16;
+    if (i >= nv) return;
+    bool bad = false;
+    if (i + 16 <= nv && (((uintptr_t)(mat + i)) & 15) == 0) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(mat + i);
+        const unsigned w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) bad |= (int)((w[e] >> (8 * b)) & 0xffu) >= n_mat;
+    } else {
+        for (size_t t = i; t < nv && t < i + 16; ++t) bad |= (int)mat[t] >= n_mat;
+    }
+    if (bad) atomicExch(errflag, 1);
+}
+}  // namespace
+
+cudaError_t dos_launch_validate_material(size_t nv, const uint8_t *mat, int n_mat, int *errflag, cudaStream_t st)
+{
+    const size_t n = (nv + 15) / 16;
+    validate_material_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(nv, mat, n_mat, errflag);
+    return cudaGetLastError();
+}
+
 cudaError_t dos_launch_fluence(size_t nv, int G, int MP, const float *phi_u, const float *phi_all, float *phi_c_out,
                                float *phi_tot_out, cudaStream_t st)
 {
@@ -385,8 +413,7 @@ cudaError_t dos_launch_fluence(size_t nv, int G, int MP, const float *phi_u, con
 cudaError_t dos_launch_dose(size_t nv, const uint8_t *mat, int n_mat, int G, int MP, const float *kerma,
                             const float *phi_u, const float *phi_all, float *dose, int accumulate, cudaStream_t st)
 {
-    (void)n_mat;
     const unsigned grid = (unsigned)((nv + 255) / 256);
-    dose_kernel<<<grid, 256, 0, st>>>(nv, mat, G, MP, kerma, phi_u, phi_all, dose, accumulate);
+    dose_kernel<<<grid, 256, 0, st>>>(nv, mat, n_mat, G, MP, kerma, phi_u, phi_all, dose, accumulate);
     return cudaGetLastError();
 }

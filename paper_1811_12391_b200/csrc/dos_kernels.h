@@ -14,15 +14,20 @@ struct SourceDev {
     int isotropic;
 };
 
+#define DOS_MAX_G 64        // energy groups (the spectrum travels in the ray-trace kernel's parameters)
+struct SpectrumDev {
+    double s[DOS_MAX_G];
+};
+
 // a1: phi_u[g][cell] = S_g exp(-tau_g)/(4 pi r^2) inside the beam (fp64 inside, fp32 store).
-// sig_t_gm [G][n_mat]; spectrum (double) [G]; errflag[0] set if a material id >= n_mat is met.
+// sig_t_gm [G][n_mat]; spectrum by value (no host buffer has to outlive the call); errflag[0] set if a material id >= n_mat is met.
 cudaError_t dos_launch_raytrace(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int n_mat, int G,
-                                const float *sig_t_gm, const double *spectrum, float *phi_u, int *errflag,
+                                const float *sig_t_gm, const SpectrumDev &spectrum, float *phi_u, int *errflag,
                                 cudaStream_t st);
 
 // a2 + a3: Q_fix[cell][lm] = Y_lm(Omega_r) sum_{g'<=g} sig_s[m][l][g'->g] phi_u[g'] +
 //                            sum_{g_lo<=g'<g} sig_s[m][l][g'->g] phi_all[g'][cell][lm]
-cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int G, int n_leg,
+cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const uint8_t *mat, int n_mat, int G, int n_leg,
                                     int L, int g, int g_lo, const float *sig_s, const float *phi_u,
                                     const float *um /* [G][Nv][MP] summed-source mode, else null */,
                                     const float *phi_all, float *qfix, cudaStream_t st);
@@ -33,7 +38,7 @@ cudaError_t dos_launch_um_accumulate(const MeshDev &m, const SourceDev &s, int G
 
 // a4: Q = Q_fix + sig_s[m][l][g->g] phi (phi ignored when first != 0); phi = 0; also clears the sweep's
 // flags (n_flags ints at `done`) and its queue head.
-cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int G, int n_leg, int L, int g,
+cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int n_mat, int G, int n_leg, int L, int g,
                                      const float *sig_s, const float *qfix, float *phi, float *q, int first,
                                      int *done, int n_flags, int *queue, cudaStream_t st);
 
@@ -43,3 +48,6 @@ cudaError_t dos_launch_fluence(size_t nv, int G, int MP, const float *phi_u, con
 cudaError_t dos_launch_dose(size_t nv, const uint8_t *mat, int n_mat, int G, int MP, const float *kerma,
                             const float *phi_u, const float *phi_all, float *dose, int accumulate,
                             cudaStream_t st);
+
+// errflag[0] = 1 if any material id of the grid is >= n_mat (run once per grid)
+cudaError_t dos_launch_validate_material(size_t nv, const uint8_t *mat, int n_mat, int *errflag, cudaStream_t st);

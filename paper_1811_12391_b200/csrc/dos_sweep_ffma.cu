@@ -1,7 +1,5 @@
-// dos_sweep_ffma.cu -- the sweep with both contractions on the FP32 pipe (FFMA); used for quadrature / P_L
-// combinations of few moments per cell (MP <= 16), where the tensor-core version (dos_sweep.cu: same work items,
-// warp roles, staging and hand-off) measures slower: at S8/P3 an 8-wide MMA tile is 37 % padding and the MMA
-// chain is longer than the 16-term FFMA chains. Option "sweep_contraction" forces either.
+// dos_sweep_ffma.cu -- the sweep with both contractions on the FP32 pipe (FFMA): the fallback for quadratures the
+// tensor-memory sweep (dos_sweep_umma.cu) has no shape for, and the A/B partner of it (option "sweep_contraction" = 1).
 //
 // The S_N transport sweep (eq. 2-3) for one group and one source
 // iteration: moment-to-discrete (a5), diamond-difference cell update with set-to-zero fixup and
@@ -86,21 +84,6 @@ __device__ __forceinline__ float4 lds_v4(unsigned a)
 }
 __device__ __forceinline__ void sts_f32(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void sts_s32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
-
-// Optional per-step timeline of one work item (option "sweep_trace_item"): every warp's lane 0 stores the SM
-// clock when it starts a step (0), after its staging / M2D phase (1), after its D2M / diamond-difference phase (2)
-// and when it reaches the step's barrier (3): trace[(step * 32 + warp) * 4 + k].
-#ifndef DOS_SWEEP_TRACE
-#define DOS_SWEEP_TRACE 0
-#endif
-__device__ __forceinline__ void trace_mark(long long *trace, int step, int warp, int which)
-{
-#if DOS_SWEEP_TRACE
-    if (trace && (threadIdx.x & 31) == 0) trace[(step * 32 + warp) * 4 + which] = clock64();
-#else
-    (void)trace; (void)step; (void)warp; (void)which;
-#endif
-}
 
 // barrier of the compute warps only (the service warp never joins it)
 __device__ __forceinline__ void bar_compute(int n_threads) { asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory"); }
@@ -265,7 +248,6 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
         g.fy_in = p.fy + (g.has_y ? (size_t)(g.id - p.a_split) * fstride_y : 0);
         g.fz_in = p.fz + (g.has_z ? (size_t)(g.id - p.ntj * p.a_split) * fstride_z : 0);
         const int o = g.o;
-        long long *const trace = (p.trace && g.id == p.trace_item) ? p.trace : nullptr;
         if (o * 8 + part != cur_oct) {
             // tables of this CTA's angles: [o][part * A, (part + 1) * A)
             const size_t abase = (size_t)o * p.per_oct_full + (size_t)part * A;
@@ -349,7 +331,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
             const uint8_t *mat_p = p.mat + cbase + 3 * istep;            // material of step t + 3
             const unsigned mat_w = smem_addr(s_mat + lane);
             auto mat_of = [&](int s, const uint8_t *q) -> int {
-                return ((unsigned)(s - t_lo) < (unsigned)nx) ? (int)__ldg(q) : 0;
+                return ((unsigned)(s - t_lo) < (unsigned)nx) ? min((int)__ldg(q), p.n_mat - 1) : 0;
             };
             __syncthreads();                          // S2: s_done, s_allowed in place
             int allowed_c = -1;
@@ -377,13 +359,11 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
             bar_compute(NB);                          // S3: step 0's staged data visible to every warp
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
-                trace_mark(trace, t, warp, 0);
                 issue_round(t);
                 sts_s32(mat_w + ((t + 2) & 3) * 128, reg_m);
                 reg_m = mat_of(t + 3, mat_p);
                 mat_p += istep;
                 cp_async_wait<DF - 1>();              // step t + 1's faces complete (this thread's copies)
-                trace_mark(trace, t, warp, 3);
                 bar_compute(NB);                      // B_t: ... visible to all; every face store of step t precedes it
                 if (lane == 0) st_release_cta(&s_done, t + 1);
             }
@@ -419,9 +399,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
 
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
-                trace_mark(trace, t, warp, 0);
                 issue_round(t);
-                trace_mark(trace, t, warp, 1);
                 // D2M of step t - 1: sum over all angles of the octant, one red per (cell, 4 moments)
                 if (t > 0 && (unsigned)(t - 1 - t_lo) < (unsigned)nx) {
                     const unsigned ps = psi_r + ((t - 1) & 1) * psi_slot;
@@ -441,9 +419,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
                     }
                 }
                 phi_p += phi_inc;
-                trace_mark(trace, t, warp, 2);
                 cp_async_wait<DF - 1>();              // step t + 1's staged data complete (this thread's copies)
-                trace_mark(trace, t, warp, 3);
                 bar_compute(NB);                      // B_t: ... and visible to all
             }
             if ((unsigned)(T - 1 - t_lo) < (unsigned)nx) {
@@ -504,7 +480,6 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
 #pragma unroll 1
         for (int t = 0; t < T; ++t) {
             // moment-to-discrete for this lane's cell, AG angles; four partial sums keep the FMA chains short
-            trace_mark(trace, t, warp, 0);
             const bool act = (unsigned)(t - t_lo) < (unsigned)nx;
             const int m0 = lds_s32(mat_r + (t & 3) * 128);
             float q[AG];
@@ -528,8 +503,6 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
 #pragma unroll
                 for (int r = 0; r < AG; ++r) q[r] = (part[r][0] + part[r][1]) + (part[r][2] + part[r][3]);
             }
-
-            trace_mark(trace, t, warp, 1);
             // inflow, diamond difference, outflow
             const unsigned fslot = (t & (RF - 1)) * fin_slot;
             const unsigned pso = psi_w + (t & 1) * psi_slot;
@@ -556,8 +529,6 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
                 sts_f32(pso + r * 128, pc);
             }
             fy_st += fy_inc; fz_st += fz_inc;
-            trace_mark(trace, t, warp, 2);
-            trace_mark(trace, t, warp, 3);
             bar_compute(NB);                          // B_t
         }
     }
@@ -593,15 +564,13 @@ static sweep_fn pick_ag(int ag, int var)
     return nullptr;
 }
 
-static int g_two_per_sm = 1;     // 1: variant 2 from 4 work items per SM, 2: whenever there are more items than SMs, 0: never
-void dos_sweep_ffma_set_two_per_sm(int on) { g_two_per_sm = on; }
-
-static sweep_fn pick(int L, int ag, int per_oct, int n_aux, int n_items)
+// two_per_sm: 1: variant 2 from 4 work items per SM, 2: whenever there are more items than SMs, 0: never (per context)
+static sweep_fn pick(int L, int ag, int per_oct, int n_aux, int n_items, int two_per_sm)
 {
     const int warps = per_oct / ag + n_aux + 2, MP = dos_mpad(L);
     int sms = 148, dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int var = warps > 16 ? 1 : ((g_two_per_sm && MP <= 16 && (g_two_per_sm == 2 ? n_items > sms : n_items >= 4 * sms)) ? 2 : 0);
+    const int var = warps > 16 ? 1 : ((two_per_sm && MP <= 16 && (two_per_sm == 2 ? n_items > sms : n_items >= 4 * sms)) ? 2 : 0);
     switch (MP) {
         case 4: return pick_ag<4>(ag, var);
         case 12: return pick_ag<12>(ag, var);
@@ -646,9 +615,9 @@ int dos_sweep_ffma_angles_per_warp(int per_oct, int L, int prefer)
     return 0;
 }
 
-cudaError_t dos_sweep_ffma_grid(int L, int ag, int n_aux, int per_oct, int n_mat, int n_items, int *grid_out)
+cudaError_t dos_sweep_ffma_grid(int L, int ag, int n_aux, int per_oct, int n_mat, int n_items, int two_per_sm, int *grid_out)
 {
-    sweep_fn f = pick(L, ag, per_oct, n_aux, n_items);
+    sweep_fn f = pick(L, ag, per_oct, n_aux, n_items, two_per_sm);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, per_oct, n_mat);
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -666,9 +635,9 @@ cudaError_t dos_sweep_ffma_grid(int L, int ag, int n_aux, int per_oct, int n_mat
     return cudaSuccess;
 }
 
-cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ag, int grid, cudaStream_t s)
+cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ag, int grid, int two_per_sm, cudaStream_t s)
 {
-    sweep_fn f = pick(L, ag, a.per_oct, a.n_aux, a.n_items);
+    sweep_fn f = pick(L, ag, a.per_oct, a.n_aux, a.n_items, two_per_sm);
     if (!f) return cudaErrorInvalidValue;
     const size_t smem = sweep_smem(L, a.per_oct, a.n_mat);
     f<<<grid, (a.n_warps + a.n_aux + 2) * 32, smem, s>>>(a);

@@ -20,10 +20,9 @@ DOS_OK = 0
 STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_ERR_STATE", -4: "DOS_ERR_NOMEM",
           -5: "DOS_ERR_CUDA", -6: "DOS_ERR_UNSUPPORTED"}
 
-EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_sum", "dos_solve",
-           "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option", "dos_profile", "dos_profile_reset",
-           "dos_sweep_trace_host",
-           "dos_destroy", "dos_last_error"]
+EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_sum",
+           "dos_uncollided_total", "dos_solve", "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option",
+           "dos_profile", "dos_profile_reset", "dos_destroy", "dos_last_error"]
 
 
 class dos_mesh(C.Structure):
@@ -78,8 +77,8 @@ _lib.dos_profile.restype = C.c_int
 _lib.dos_profile.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dos_profile_reset.restype = C.c_int
 _lib.dos_profile_reset.argtypes = [C.c_void_p]
-_lib.dos_sweep_trace_host.restype = C.c_int
-_lib.dos_sweep_trace_host.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+_lib.dos_uncollided_total.restype = C.c_int
+_lib.dos_uncollided_total.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dos_destroy.restype = None
 _lib.dos_destroy.argtypes = [C.c_void_p]
 _lib.dos_last_error.restype = C.c_char_p
@@ -194,6 +193,9 @@ class Context:
         ptr = phi_u_out.data_ptr() if phi_u_out is not None else None
         self._check(_lib.dos_uncollided_sum(self.handle, C.byref(src), sp.ctypes.data, int(bool(first)), ptr))
 
+    def dos_uncollided_total(self, phi_u_out):
+        self._check(_lib.dos_uncollided_total(self.handle, phi_u_out.data_ptr()))
+
     def dos_solve(self, n_iter):
         self._check(_lib.dos_solve(self.handle, int(n_iter)))
 
@@ -219,13 +221,6 @@ class Context:
         self._check(_lib.dos_profile(self.handle, C.byref(p)))
         return {"sweep_ms": p.sweep_ms, "sweep_launches": p.sweep_launches, "raytrace_ms": p.raytrace_ms,
                 "raytrace_launches": p.raytrace_launches, "kernel_launches": p.kernel_launches}
-
-    def dos_sweep_trace_host(self):
-        """[steps][32 warps][4] int64 SM clocks of the traced sweep item (option sweep_trace_item)."""
-        steps = self.mesh["nx"] + 10
-        buf = np.zeros((steps, 32, 4), dtype=np.int64)
-        self._check(_lib.dos_sweep_trace_host(self.handle, buf.ctypes.data, buf.size))
-        return buf
 
     def dos_profile_reset(self):
         self._check(_lib.dos_profile_reset(self.handle))
@@ -272,11 +267,9 @@ def run_problem_summed(p, source_indices=None, n_iter=None, device="cuda:0"):
     ctx = Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"],
                   device=device, n_batch=max(2, len(idx)))
     pu, pc, pt, d = ctx.new_field(), ctx.new_field(), ctx.new_field(), ctx.new_field(groups=False)
-    one = ctx.new_field()
-    pu.zero_()
     for n, s in enumerate(idx):
-        ctx.dos_uncollided_sum(p["sources"][s], p["spectrum"], first=(n == 0), phi_u_out=one)
-        pu += one                                   # bookkeeping of the return value only; the library keeps its own sum
+        ctx.dos_uncollided_sum(p["sources"][s], p["spectrum"], first=(n == 0))
+    ctx.dos_uncollided_total(pu)                    # the library's own sum over the positions
     ctx.dos_solve(p["n_iter"] if n_iter is None else n_iter)
     ctx.dos_fluence(pc, pt)
     ctx.dos_dose(d, False)

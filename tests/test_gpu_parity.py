@@ -54,15 +54,14 @@ def test_small_problem_parity(dos, orc, name, ov):
     assert_problem_parity(out, ref, name)
 
 
-# Every sweep implementation on every kind of problem, whatever the library's default choice is: FFMA contractions
-# (dos_sweep_ffma.cu), tensor-core contractions (dos_sweep.cu), the 64-register two-CTAs-per-SM variants, 8 aux warps.
+# Every sweep implementation on every kind of problem, whatever the library's default choice is: the tensor-memory sweep
+# (dos_sweep_umma.cu: tcgen05.mma contractions, bulk copies, mbarrier rings), also with an odd hand-off chunk and few
+# persistent CTAs, and the FFMA sweep (dos_sweep_ffma.cu) with and without its two-CTAs-per-SM variant.
 SWEEP_VARIANTS = [
+    ("umma", {"sweep_contraction": 2}),
+    ("umma-chunk3-grid5", {"sweep_contraction": 2, "sweep_chunk": 3, "sweep_grid": 5}),
     ("ffma", {"sweep_contraction": 1, "sweep_two_per_sm": 0}),
-    ("ffma-2cta", {"sweep_contraction": 1, "sweep_two_per_sm": 6}),
-    ("mma", {"sweep_contraction": 2, "sweep_two_per_sm": 0}),
-    ("mma-2cta", {"sweep_contraction": 2, "sweep_two_per_sm": 1}),
-    ("mma-8aux", {"sweep_contraction": 2, "sweep_aux_warps": 8}),
-    ("v1", {"sweep_impl": 1}),
+    ("ffma-2cta", {"sweep_contraction": 1, "sweep_two_per_sm": 2}),
 ]
 VARIANT_CASES = [
     ("config2", dict(nx=37, ny=21, nz=10, voxel=1.0, n_group=4, n_iter=4)),                        # S8/P3, ragged tiles
@@ -79,19 +78,13 @@ def test_every_sweep_variant_parity(dos, orc, case):
     name, ov = VARIANT_CASES[case]
     p = _make(name, **ov)
     ref = orc.run_problem(p)
-    try:
-        for label, opts in SWEEP_VARIANTS:
-            ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
-            for k, v in opts.items():
-                ctx.dos_set_option(k, v)
-            out = dos.run_problem(p, ctx=ctx)
-            ctx.close()
-            assert_problem_parity(out, ref, f"{name} [{label}]")
-    finally:
-        # sweep_two_per_sm is process-wide: back to the library default
+    for label, opts in SWEEP_VARIANTS:
         ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
-        ctx.dos_set_option("sweep_two_per_sm", 2)
+        for k, v in opts.items():
+            ctx.dos_set_option(k, v)
+        out = dos.run_problem(p, ctx=ctx)
         ctx.close()
+        assert_problem_parity(out, ref, f"{name} [{label}]")
 
 
 def test_summed_source_mode_parity(dos, orc):
