@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SOURCES = ["dos_api.cu", "dos_kernels.cu", "dos_sweep_umma.cu", "dos_sweep_ffma.cu"]
 HEADERS = ["dos_internal.h", "dos_kernels.h", "dos_sm100.cuh", os.path.join("..", "..", "include", "dos.h")]
 LIB = os.path.join(HERE, "libdos.so")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++20", "-Xcompiler", "-fPIC"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -23,6 +23,31 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, unsigned by
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// Up to `tries` polls in a three-instruction loop; each poll may suspend the thread for up to ~`hint_ns` (the
+// hardware wakes it when the phase completes), so a waiting warp costs next to no issue slots. Returns 1 on success.
+__device__ __forceinline__ unsigned mbar_wait_some(uint64_t *bar, unsigned parity, unsigned tries, unsigned hint_ns)
+{
+    unsigned ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .u32 n;\n\tmov.u32 n, %3;\n"
+        "W_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %4;\n\t@p bra D_%=;\n\t"
+        "sub.u32 n, n, 1;\n\tsetp.ne.u32 p, n, 0;\n\t@p bra W_%=;\n\tmov.u32 %0, 0;\n\tbra E_%=;\n"
+        "D_%=:\n\tmov.u32 %0, 1;\nE_%=:\n\t}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(tries), "r"(hint_ns)
+        : "memory");
+    return ok;
+}
+// 16-byte asynchronous copy global -> shared that bypasses L1 (LDGSTS) and an mbarrier arrival that fires when all of
+// this thread's earlier cp.async have landed (no increment of the pending count: the init count covers it)
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive(uint64_t *bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, unsigned parity)
 {
     unsigned ok;
@@ -164,11 +189,35 @@ __device__ __forceinline__ void umma_ts(unsigned d_tmem, unsigned a_tmem, uint64
                  "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
                  : "memory");
 }
+// The same, issued under a predicate INSIDE the asm block (`on` is true in exactly one lane of a converged warp): a C++
+// `if (leader)` around a uniform-datapath instruction makes the compiler wrap it in an ELECT / BRA.U.ANY loop.
+__device__ __forceinline__ void umma_ss_if(unsigned on, unsigned d_tmem, uint64_t a_desc, uint64_t b_desc, unsigned idesc, unsigned accumulate)
+{
+    asm volatile("{\n\t.reg .pred p, e;\n\tsetp.ne.b32 e, %5, 0;\n\tsetp.ne.b32 p, %4, 0;\n\t@e tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(d_tmem),
+                 "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(on)
+                 : "memory");
+}
+__device__ __forceinline__ void umma_ts_if(unsigned on, unsigned d_tmem, unsigned a_tmem, uint64_t b_desc, unsigned idesc, unsigned accumulate)
+{
+    asm volatile("{\n\t.reg .pred p, e;\n\tsetp.ne.b32 e, %5, 0;\n\tsetp.ne.b32 p, %4, 0;\n\t@e tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}\n" ::"r"(d_tmem),
+                 "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(on)
+                 : "memory");
+}
+__device__ __forceinline__ void umma_commit_if(unsigned on, uint64_t *bar)
+{
+    asm volatile("{\n\t.reg .pred e;\n\tsetp.ne.b32 e, %1, 0;\n\t@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}\n" ::"r"(smem_u32(bar)), "r"(on)
+                 : "memory");
+}
 // the mbarrier gets one arrival when every tcgen05.mma issued so far by this thread has completed
 __device__ __forceinline__ void umma_commit(uint64_t *bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// warp-group register re-allocation (all warps of an aligned group of 4 must execute the same one)
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ bool elect_one()
 {
     unsigned e;

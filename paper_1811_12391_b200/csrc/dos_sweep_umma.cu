@@ -25,6 +25,8 @@
 //               by wavefront diagonal, published every `chunk` steps by the service warp (st.release.gpu), acquired by
 //               the downwind CTA's service warp, staged by its feeder warp with bulk copies.
 // The angular flux never leaves registers / tensor memory.
+#include <utility>
+
 #include "dos_internal.h"
 #include "dos_sm100.cuh"
 
@@ -40,7 +42,18 @@ constexpr int PSL = 2;       // ring of psi operands (hi, lo) in TMEM
 constexpr int DPS = 2;       // ring of D2M accumulators in TMEM
 constexpr int RFU = 4;       // ring of staged tile-inflow faces (steps)
 constexpr int BIG = 1 << 30;
-constexpr int WAIT_LIMIT = 1 << 22;
+constexpr int WAIT_LIMIT = 1 << 24;     // sleeping polls (>= 64 ns each: seconds) before a wait declares the launch stuck
+#ifndef DOS_UMMA_TRACE
+#define DOS_UMMA_TRACE 0      // measurement builds only: SM-clock timeline of one work item into the face buffer's tail
+#endif
+#if DOS_UMMA_TRACE
+#define TRACE(ev) do { if (trace_on && lane == 0 && t >= 100 && t < 164) trace_buf[((warp * 64 + (t - 100)) * 8) + (ev)] = clock64(); } while (0)
+#else
+#define TRACE(ev) do { } while (0)
+#endif
+#ifndef DOS_UMMA_ABL
+#define DOS_UMMA_ABL 0        // measurement builds only: bit 0 no source-moment copies, 1 no reds, 2 no MMAs, 3 no cell update
+#endif
 
 __device__ __forceinline__ int ld_relaxed_gpu(const int *p)
 {
@@ -65,21 +78,22 @@ __device__ __forceinline__ void red_add_v4(float *p, float a, float b, float c, 
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
-// Bounded wait on an mbarrier phase. A hand-off that never arrives must not hang the GPU: the waiter sets the CTA's
-// and the launch's abort flags and everything drains with invalid results (dos_check then reports DOS_ERR_CUDA).
-__device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_abort, int *g_abort)
+// Bounded wait on an mbarrier phase. A waiting warp must not spend issue slots: measured, try_wait returns within
+// ~50 cycles whether or not it carries a suspend-time hint, and twelve helper warps polling back to back issued more
+// instructions than the sixteen compute warps doing the work. So: one poll, then sleep between polls.
+// A hand-off that never arrives must not hang the GPU: the waiter sets the CTA's and the launch's abort flags and
+// everything drains with invalid results (dos_check then reports DOS_ERR_CUDA).
+__device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_abort, int *g_abort, unsigned sleep_ns = 64)
 {
     if (mbar_try_wait(bar, parity)) return;
-    int spins = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        ++spins;
-        if ((spins & 255) == 0 && *(volatile int *)s_abort) return;
-        if (spins > WAIT_LIMIT) {
-            *(volatile int *)s_abort = 1;
-            atomicExch(g_abort, 1);
-            return;
-        }
+#pragma unroll 1
+    for (int spins = 0; spins < WAIT_LIMIT; ++spins) {
+        __nanosleep(sleep_ns);
+        if (mbar_try_wait(bar, parity)) return;
+        if ((spins & 1023) == 1023 && *(volatile int *)s_abort) return;
     }
+    *(volatile int *)s_abort = 1;
+    atomicExch(g_abort, 1);
 }
 
 // Slow path of the cell update: at least one extrapolated outflow was negative. Faces found negative are pinned to
@@ -109,6 +123,9 @@ __device__ __forceinline__ void tf32_split(float x, float &hi, float &lo)
     lo = x - hi;
 }
 
+__host__ __device__ constexpr int umma_reg_compute(int ng) { return ng == 4 ? 96 : 120; }
+__host__ __device__ constexpr int umma_reg_helper(int) { return 40; }
+
 struct Geom {          // one octant's (j,k) column of this lane
     bool valid;
     int t_lo;          // first active step (skew), BIG if the column is outside the mesh
@@ -129,16 +146,16 @@ __device__ __forceinline__ Geom make_geom(const SweepUArgs &p, int o, int tj, in
     return g;
 }
 
-// Epilogue of one row: D_phi columns [C0, MP) -> mirror signs -> phi[cell][C0..MP) by red.global.add.v4, 16 columns at a time.
+// Epilogue of one row: D_phi columns [C0, MP) -> mirror signs -> phi[cell][C0..MP) by red.global.add.v4, 8 columns at a time.
 template <int MP, int C0>
 __device__ __forceinline__ void epilogue_row(unsigned taddr, const unsigned *sgn, float *phi, bool on)
 {
     if constexpr (C0 < MP) {
-        constexpr int N = MP - C0 < 16 ? MP - C0 : 16;
+        constexpr int N = MP - C0 < 8 ? MP - C0 : 8;
         float v[N];
         tmem_ld_n<N>(taddr + C0, v);
         tmem_wait_ld();
-        if (on) {
+        if (on && !(DOS_UMMA_ABL & 2)) {
 #pragma unroll
             for (int e = 0; e < N; e += 4) {
                 const uint4 s = *reinterpret_cast<const uint4 *>(sgn + C0 + e);
@@ -147,6 +164,37 @@ __device__ __forceinline__ void epilogue_row(unsigned taddr, const unsigned *sgn
             }
         }
         epilogue_row<MP, C0 + N>(taddr, sgn, phi, on);
+    }
+}
+
+// Split warp, one row of NQ float4: stage (cp.async) and convert (mirror signs, TF32 hi / lo, UMMA core-matrix layout).
+template <int NQ>
+__device__ __forceinline__ void split_issue(float *dst, const float *src)
+{
+#pragma unroll
+    for (int c = 0; c < NQ; ++c) cp_async16(dst + 4 * c, src + 4 * c);
+}
+template <int NQ>
+__device__ __forceinline__ void split_row(const float4 *src, const unsigned *sgn, float4 *dh, float4 *dl, bool on)
+{
+#pragma unroll
+    for (int b = 0; b < NQ; b += 3) {                 // 3 float4 in flight: the helper warps live in 40 registers
+        float4 x[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            if (b + c < NQ) x[c] = on ? src[b + c] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            if (b + c < NQ) {
+                const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn + 4 * (b + c));
+                float4 h, l;
+                tf32_split(__uint_as_float(__float_as_uint(x[c].x) ^ s4.x), h.x, l.x);
+                tf32_split(__uint_as_float(__float_as_uint(x[c].y) ^ s4.y), h.y, l.y);
+                tf32_split(__uint_as_float(__float_as_uint(x[c].z) ^ s4.z), h.z, l.z);
+                tf32_split(__uint_as_float(__float_as_uint(x[c].w) ^ s4.w), h.w, l.w);
+                dh[(b + c) * 8] = h;
+                dl[(b + c) * 8] = l;
+            }
     }
 }
 
@@ -205,7 +253,7 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
     for (int i = tid; i < p.n_mat; i += blockDim.x) s_sig[i] = p.sig_t[i];
     for (int i = tid; i < 8 * MP; i += blockDim.x) s_sign[i] = p.signs[i];
     if (tid == 0) {
-        for (int i = 0; i < 16; ++i) mbar_init(&raw_full[i], 1);
+        for (int i = 0; i < 16; ++i) mbar_init(&raw_full[i], 32);
         for (int i = 0; i < ASL; ++i) { mbar_init(&a_full[i], 4); mbar_init(&a_empty[i], 1); }
         for (int i = 0; i < DQS; ++i) { mbar_init(&q_full[i], 1); mbar_init(&q_empty[i], NCW); }
         for (int i = 0; i < PSL; ++i) { mbar_init(&psi_full[i], NCW); mbar_init(&psi_empty[i], 1); }
@@ -236,19 +284,41 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
 
     unsigned gs0 = 0;      // global step counter at the start of the current item (ring slots and phases follow it)
     unsigned fs0 = 0;      // the same for the tile-inflow ring, which only items with an upwind tile use
-    for (;;) {
+    // Every role runs its own loop over the work items (so that each role's code lies behind its own setmaxnreg and
+    // ptxas can give it its own register budget); all of them meet in the two barriers of next_item().
+    int quad = 0, tj = 0, tk = 0, fid = 0;
+    bool has_y = false, has_z = false;
+#if DOS_UMMA_TRACE
+    bool trace_on = false;
+    long long *trace_buf = reinterpret_cast<long long *>(p.fz);      // measurement build: the z-face buffer of item 0 is sacrificed
+#endif
+    auto next_item = [&]() -> bool {
         __syncthreads();                              // every role has drained the previous item
         if (tid == 0) s_item = atomicAdd(p.queue, 1);
         if (tid < NCW) s_prog[tid] = 0;
         __syncthreads();
         const int item = s_item;
-        if (item >= p.n_items) break;
+        if (item >= p.n_items) return false;
         const int packed = p.items[item];
-        const int quad = packed & 7, tj = (packed >> 3) & 0x3FFF, tk = packed >> 17;
-        const int fid = (quad * p.ntk + tk) * p.ntj + tj;            // hand-off flag of this (quad, tile)
-        const bool has_y = tj > 0, has_z = tk > 0;
+        quad = packed & 7; tj = (packed >> 3) & 0x3FFF; tk = packed >> 17;
+        fid = (quad * p.ntk + tk) * p.ntj + tj;      // hand-off flag of this (quad, tile)
+        has_y = tj > 0; has_z = tk > 0;
+#if DOS_UMMA_TRACE
+        trace_on = item == 601;
+#endif
+        return true;
+    };
+    // Register re-allocation (warp roles come in aligned groups of 4 warps, as setmaxnreg requires): the compute warps
+    // carry 3 face fluxes per angle plus the cell update's temporaries, the helper warps need little.
+    // setmaxnreg re-divides the CTA's OWN register allocation (threads x registers at launch), it cannot draw on the
+    // rest of the register file: with more than the launch total the increase blocks for ever. NG = 4: 896 threads x 72 =
+    // 16 warps x 96 + 12 x 40; NG = 3: 768 x 80 = 12 x 120 + 12 x 40 (dos_sweep_umma_grid checks the launch count).
+    constexpr int REG_C = umma_reg_compute(NG), REG_H = umma_reg_helper(NG);
+    constexpr bool REALLOC = NG >= 3;
 
-        if (is_service) {
+    if (is_service) {
+        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+        while (next_item()) {
             // ------- service warp: publishes this item's progress, follows the two upwind items' progress -------
             const int *up_y = p.done + (has_y ? fid - 1 : fid), *up_z = p.done + (has_z ? fid - p.ntj : fid);
             int *my_flag = p.done + fid;
@@ -288,10 +358,10 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                 }
             }
             gs0 += T;
-            continue;
         }
-
-        if (is_feed) {
+    } else if (is_feed) {
+        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+        while (next_item()) {
             // ------- feeder warp: bulk copies of the tile-inflow faces the upwind tiles have published -------
             // step s of octant qq needs fy_in[s][A][TK] and fz_in[s][A][TJ]: two contiguous blocks per octant.
             __syncthreads();                          // S2: s_allowed in place
@@ -329,10 +399,10 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                 fs0 += T;
             }
             gs0 += T;
-            continue;
         }
-
-        if (is_m2d) {
+    } else if (is_m2d) {
+        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+        while (next_item()) {
             // ------- M2D issuer: D_q[slot] = A_lo B_hi + A_hi B_lo + A_hi B_hi -------
             __syncthreads();                          // S2
             const bool leader = elect_one();
@@ -342,27 +412,32 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
+                TRACE(0);
                 wait_bar(&a_full[gs % ASL], (gs / ASL) & 1, &s_abort, p.abort_flag);
+                TRACE(1);
                 wait_bar(&q_empty[gs % DQS], ((gs / DQS) & 1) ^ 1, &s_abort, p.abort_flag);
+                TRACE(2);
                 tc_fence_after();
-                if (leader) {
+                {
+                    const unsigned on = (leader && !(DOS_UMMA_ABL & 4)) ? 1u : 0u;
                     const unsigned a0 = smem_u32(s_a) + (gs % ASL) * a_slot_bytes;
                     const uint64_t adh = umma_smem_desc(a0, 128, NCH * 128), adl = umma_smem_desc(a0 + a_half, 128, NCH * 128);
                     const unsigned d = tm_dq + (gs % DQS) * NAP;
-                    unsigned acc = 0;
-                    for (int ks = 0; ks < KP / 8; ++ks) { umma_ss(d, adl + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, acc); acc = 1; }
-                    for (int ks = 0; ks < KP / 8; ++ks) umma_ss(d, adh + (uint64_t)(ks * 16), bdl + (uint64_t)(ks * 16), idesc, 1);
-                    for (int ks = 0; ks < KP / 8; ++ks) umma_ss(d, adh + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, 1);
-                    umma_commit(&q_full[gs % DQS]);
-                    umma_commit(&a_empty[gs % ASL]);
+                    const int nk = KP / 8;
+                    for (int ks = 0; ks < nk; ++ks) umma_ss_if(on, d, adl + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, ks ? 1u : 0u);
+                    for (int ks = 0; ks < nk; ++ks) umma_ss_if(on, d, adh + (uint64_t)(ks * 16), bdl + (uint64_t)(ks * 16), idesc, 1u);
+                    for (int ks = 0; ks < nk; ++ks) umma_ss_if(on, d, adh + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, 1u);
+                    umma_commit_if(leader ? 1u : 0u, &q_full[gs % DQS]);
+                    umma_commit_if(leader ? 1u : 0u, &a_empty[gs % ASL]);
                 }
                 __syncwarp();
+                TRACE(3);
             }
             gs0 += T;
-            continue;
         }
-
-        if (is_d2m) {
+    } else if (is_d2m) {
+        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+        while (next_item()) {
             // ------- D2M issuer: D_phi[slot] = psi_lo B_hi + psi_hi B_lo + psi_hi B_hi (A operand in TMEM) -------
             __syncthreads();                          // S2
             const bool leader = elect_one();
@@ -372,31 +447,35 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
+                TRACE(0);
                 wait_bar(&psi_full[gs % PSL], (gs / PSL) & 1, &s_abort, p.abort_flag);
+                TRACE(1);
                 wait_bar(&phi_empty[gs % DPS], ((gs / DPS) & 1) ^ 1, &s_abort, p.abort_flag);
+                TRACE(2);
                 tc_fence_after();
-                if (leader) {
+                {
+                    const unsigned on = (leader && !(DOS_UMMA_ABL & 4)) ? 1u : 0u;
                     const unsigned ah = tm_psi + (gs % PSL) * 2 * A8, al = ah + A8;
                     const unsigned d = tm_dphi + (gs % DPS) * NMP;
-                    unsigned acc = 0;
-                    for (int ks = 0; ks < A8 / 8; ++ks) { umma_ts(d, al + ks * 8, bdh + (uint64_t)(ks * 16), idesc, acc); acc = 1; }
-                    for (int ks = 0; ks < A8 / 8; ++ks) umma_ts(d, ah + ks * 8, bdl + (uint64_t)(ks * 16), idesc, 1);
-                    for (int ks = 0; ks < A8 / 8; ++ks) umma_ts(d, ah + ks * 8, bdh + (uint64_t)(ks * 16), idesc, 1);
-                    umma_commit(&phi_full[gs % DPS]);
-                    umma_commit(&psi_empty[gs % PSL]);
+                    const int nk = A8 / 8;
+                    for (int ks = 0; ks < nk; ++ks) umma_ts_if(on, d, al + ks * 8, bdh + (uint64_t)(ks * 16), idesc, ks ? 1u : 0u);
+                    for (int ks = 0; ks < nk; ++ks) umma_ts_if(on, d, ah + ks * 8, bdl + (uint64_t)(ks * 16), idesc, 1u);
+                    for (int ks = 0; ks < nk; ++ks) umma_ts_if(on, d, ah + ks * 8, bdh + (uint64_t)(ks * 16), idesc, 1u);
+                    umma_commit_if(leader ? 1u : 0u, &phi_full[gs % DPS]);
+                    umma_commit_if(leader ? 1u : 0u, &psi_empty[gs % PSL]);
                 }
                 __syncwarp();
+                TRACE(3);
             }
             gs0 += T;
-            continue;
         }
-
-        // the remaining roles own octant o = 4 quad + q and this lane's (j,k) column of its tile
-        const int o = quad * 4 + q;
-        const Geom g = make_geom(p, o, tj, tk, lane);
-        const int row = q * 32 + lane;
-
-        if (is_split) {
+    } else if (is_split) {
+        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+        while (next_item()) {
+            // this warp owns octant o = 4 quad + q; the lane owns one (j,k) column of its tile
+            const int o = quad * 4 + q;
+            const Geom g = make_geom(p, o, tj, tk, lane);
+            const int row = q * 32 + lane;
             // ------- split warp: bulk copy of each row's MP source moments, mirror signs, TF32 hi / lo, UMMA layout -------
             __syncthreads();                          // S2
             const float *qsrc = p.Q + g.cbase * MP;
@@ -404,47 +483,58 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             const unsigned *sgn = s_sign + o * MP;
             const int nq = MP / 4;
             auto issue = [&](int s) {
+                // one 16-byte cp.async per 4 moments of this lane's row; the lane's arrival on the ring slot's mbarrier
+                // fires when they have landed
                 const bool on = (unsigned)(s - g.t_lo) < (unsigned)nx;
-                const unsigned m = __ballot_sync(0xffffffffu, on);
                 uint64_t *bar = &raw_full[((gs0 + s) % RAW) * 4 + q];
-                if (lane == 0) mbar_arrive_expect_tx(bar, (unsigned)__popc(m) * (unsigned)MP * 4u);
-                __syncwarp();
-                if (on) bulk_g2s(s_raw + ((size_t)((gs0 + s) % RAW) * 128 + row) * MP, qsrc + qinc * s, (unsigned)MP * 4u, bar);
+                if (on && !(DOS_UMMA_ABL & 1)) {
+                    float *dst = s_raw + ((size_t)((gs0 + s) % RAW) * 128 + row) * MP;
+                    const float *src = qsrc + qinc * s;
+                    switch (nq) {
+                        case 1: split_issue<1>(dst, src); break;
+                        case 3: split_issue<3>(dst, src); break;
+                        case 4: split_issue<4>(dst, src); break;
+                        case 7: split_issue<7>(dst, src); break;
+                        default: split_issue<9>(dst, src); break;
+                    }
+                }
+                cp_async_mbar_arrive(bar);
             };
             for (int s = 0; s < LA && s < T; ++s) issue(s);
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
+                TRACE(0);
                 if (t + LA < T) issue(t + LA);
+                TRACE(1);
                 wait_bar(&raw_full[(gs % RAW) * 4 + q], (gs / RAW) & 1, &s_abort, p.abort_flag);
+                TRACE(2);
                 wait_bar(&a_empty[gs % ASL], ((gs / ASL) & 1) ^ 1, &s_abort, p.abort_flag);
+                TRACE(3);
                 const bool on = (unsigned)(t - g.t_lo) < (unsigned)nx;
                 const float4 *src = reinterpret_cast<const float4 *>(s_raw + ((size_t)(gs % RAW) * 128 + row) * MP);
                 // element (row, chunk c): ((row / 8) * NCH + c) * 32 + (row % 8) * 4 floats
                 float4 *dh = reinterpret_cast<float4 *>(s_a + (size_t)(gs % ASL) * (2 * 16 * NCH * 32) + ((row >> 3) * NCH) * 32 + (row & 7) * 4);
                 float4 *dl = dh + 16 * NCH * 8;
-                for (int c = 0; c < nq; ++c) {
-                    float4 h = make_float4(0.f, 0.f, 0.f, 0.f), l = h;
-                    if (on) {
-                        const float4 x = src[c];
-                        const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn + 4 * c);
-                        tf32_split(__uint_as_float(__float_as_uint(x.x) ^ s4.x), h.x, l.x);
-                        tf32_split(__uint_as_float(__float_as_uint(x.y) ^ s4.y), h.y, l.y);
-                        tf32_split(__uint_as_float(__float_as_uint(x.z) ^ s4.z), h.z, l.z);
-                        tf32_split(__uint_as_float(__float_as_uint(x.w) ^ s4.w), h.w, l.w);
-                    }
-                    dh[c * 8] = h;
-                    dl[c * 8] = l;
+                switch (nq) {
+                    case 1: split_row<1>(src, sgn, dh, dl, on); break;
+                    case 3: split_row<3>(src, sgn, dh, dl, on); break;
+                    case 4: split_row<4>(src, sgn, dh, dl, on); break;
+                    case 7: split_row<7>(src, sgn, dh, dl, on); break;
+                    default: split_row<9>(src, sgn, dh, dl, on); break;
                 }
                 fence_proxy_async_smem();             // the stores above -> the UMMA's operand reads; the row reads -> the next bulk copy
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&a_full[gs % ASL]);
+                TRACE(4);
             }
             gs0 += T;
-            continue;
         }
-
-        if (is_epi) {
+    } else if (is_epi) {
+        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+        while (next_item()) {
+            const int o = quad * 4 + q;
+            const Geom g = make_geom(p, o, tj, tk, lane);
             // ------- epilogue warp: D_phi row -> mirror signs -> red.global.add into phi[cell][MP] -------
             __syncthreads();                          // S2
             float *phi_p = p.phi + g.cbase * MP;
@@ -453,7 +543,9 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
+                TRACE(0);
                 wait_bar(&phi_full[gs % DPS], (gs / DPS) & 1, &s_abort, p.abort_flag);
+                TRACE(1);
                 tc_fence_after();
                 const bool on = (unsigned)(t - g.t_lo) < (unsigned)nx;
                 const unsigned ta = tm_dphi + lane_base + (gs % DPS) * NMP;
@@ -467,14 +559,17 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&phi_empty[gs % DPS]);
+                TRACE(2);
                 phi_p += pinc;
             }
             gs0 += T;
-            continue;
         }
-
+    } else {
         // ---------------- compute warps: diamond difference, face hand-off ----------------
-        {
+        if constexpr (REALLOC) setmaxnreg_inc<REG_C>();
+        while (next_item()) {
+            const int o = quad * 4 + q;
+            const Geom g = make_geom(p, o, tj, tk, lane);
             const int grp = warp >> 2, a0 = grp * AG;
             const int jj = lane & (DOS_TJ - 1), kk = lane / DOS_TJ;
             const bool in_y = jj == 0, in_z = kk == 0;
@@ -502,59 +597,99 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                 const int m0 = m_cur;
                 m_cur = m_nxt;
                 m_nxt = mat_of(t + 2);
-                // discrete source of this lane's cell for the warp's AG angles, straight from tensor memory
-                float qd[AG];
-                wait_bar(&q_full[gs % DQS], (gs / DQS) & 1, &s_abort, p.abort_flag);
+                TRACE(0);
+                wait_bar(&q_full[gs % DQS], (gs / DQS) & 1, &s_abort, p.abort_flag, 32);
+                TRACE(1);
                 tc_fence_after();
-                tmem_ld_n<AG>(tm_dq + lane_base + (gs % DQS) * NAP + a0, qd);
-                tmem_wait_ld();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&q_empty[gs % DQS]);
                 const unsigned fs = fs0 + t;
-                if (has_y || has_z) wait_bar(&fin_full[fs % RFU], (fs / RFU) & 1, &s_abort, p.abort_flag);
+                if (has_y || has_z) wait_bar(&fin_full[fs % RFU], (fs / RFU) & 1, &s_abort, p.abort_flag, 32);
+                TRACE(3);
                 const int fslot = (int)(fs % RFU) * 4 * A;
                 const float *rden = s_rden + m0 * A + a0;
+                const float sig0 = s_sig[m0];
                 const bool first_x = t == t_lo;
-                float pc[AG];
+                const unsigned tq = tm_dq + lane_base + (gs % DQS) * NAP + a0;            // D_q columns of this warp's angles
+                const unsigned tp = tm_psi + lane_base + (gs % PSL) * 2 * A8 + a0;        // psi operand columns (hi; lo at + A8)
+                // The AG angles go in chunks of CH. Inside a chunk everything is straight-line code (selects, no branches),
+                // so the CH independent dependency chains interleave; the set-to-zero fixup runs for the whole chunk in
+                // lock-step while any lane of the warp still has a negative outflow. R12: the pinned set only grows. A
+                // pinned face has outflow exactly 0, so "pinned" is read off the outflow itself (o <= 0): a face whose
+                // unpinned outflow is exactly 0 may be treated as pinned, because pinning any other face lowers psi_c and
+                // would pin it in the next pass anyway. A pass with nothing new to pin reproduces its input.
+                // Each chunk reads its CH columns of the discrete source from tensor memory and writes its psi_c (TF32
+                // hi + lo) back as the D2M's A operand, so no per-angle array outlives a chunk except the 3 face fluxes.
+                constexpr int CH = (AG % 4 == 0 || AG == 7) ? 4 : (AG >= 3 ? 3 : AG);
+                auto chunk = [&]<int C0>() {
+                    constexpr int N = AG - C0 < CH ? AG - C0 : CH;
+                    float qd[N], ix[N], yi[N], zi[N], ox[N], oyr[N], ozr[N], pc[N];
+                    tmem_ld_n<N>(tq + C0, qd);
+                    tmem_wait_ld();
+                    bool any = false;
 #pragma unroll
-                for (int r = 0; r < AG; ++r) {
-                    float yin = __shfl_up_sync(0xffffffffu, oy[r], 1);
-                    float zin = __shfl_up_sync(0xffffffffu, oz[r], DOS_TJ);
-                    if (in_y) yin = has_y ? finy[fslot * DOS_TK + r * DOS_TK] : 0.f;        // tile inflow or vacuum
-                    if (in_z) zin = has_z ? finz[fslot * DOS_TJ + r * DOS_TJ] : 0.f;
-                    float c = 0.f;
-                    if (act) {
+                    for (int e = 0; e < N; ++e) {
+                        const int r = C0 + e;
+                        float yin = __shfl_up_sync(0xffffffffu, oy[r], 1);
+                        float zin = __shfl_up_sync(0xffffffffu, oz[r], DOS_TJ);
+                        if (in_y) yin = has_y ? finy[fslot * DOS_TK + r * DOS_TK] : 0.f;        // tile inflow or vacuum
+                        if (in_z) zin = has_z ? finz[fslot * DOS_TJ + r * DOS_TJ] : 0.f;
                         const float4 cc = cdd4[r];
-                        const float ix = first_x ? 0.f : px[r];
-                        const float num = fmaf(cc.x, ix, fmaf(cc.y, yin, fmaf(cc.z, zin, qd[r])));
-                        c = num * rden[r];
-                        float ox = 2.f * c - ix, oyr = 2.f * c - yin, ozr = 2.f * c - zin;
-                        if (fminf(ox, fminf(oyr, ozr)) < 0.f)
-                            dd_fixup(c, ox, oyr, ozr, qd[r], s_sig[m0], cc.x, cc.y, cc.z, ix, yin, zin);
-                        px[r] = ox; oy[r] = oyr; oz[r] = ozr;
-                        if (store_y) __stcg(fy_st + r * DOS_TK, oyr);
-                        if (store_z) __stcg(fz_st + r * DOS_TJ, ozr);
+                        ix[e] = first_x ? 0.f : px[r];
+                        yi[e] = yin; zi[e] = zin;
+                        const float num = fmaf(cc.x, ix[e], fmaf(cc.y, yin, fmaf(cc.z, zin, qd[e])));
+                        const float c = (DOS_UMMA_ABL & 8) ? 0.f : num * rden[r];
+                        pc[e] = c;
+                        ox[e] = 2.f * c - ix[e]; oyr[e] = 2.f * c - yin; ozr[e] = 2.f * c - zin;
+                        any |= act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
                     }
-                    pc[r] = c;
-                }
-                fy_st += fy_inc; fz_st += fz_inc;
-                // psi_c of the step, split into TF32 hi + lo, becomes the D2M's A operand in tensor memory
-                float hi[AG], lo[AG];
+                    while (__any_sync(0xffffffffu, any)) {
+                        any = false;
 #pragma unroll
-                for (int r = 0; r < AG; ++r) tf32_split(pc[r], hi[r], lo[r]);
-                wait_bar(&psi_empty[gs % PSL], ((gs / PSL) & 1) ^ 1, &s_abort, p.abort_flag);
-                tc_fence_after();
-                const unsigned tp = tm_psi + lane_base + (gs % PSL) * 2 * A8 + a0;
-                tmem_st_n<AG>(tp, hi);
-                tmem_st_n<AG>(tp + A8, lo);
+                        for (int e = 0; e < N; ++e) {
+                            const float4 cc = cdd4[C0 + e];
+                            const float gx = ox[e] > 0.f ? 1.f : 0.f, gy = oyr[e] > 0.f ? 1.f : 0.f, gz = ozr[e] > 0.f ? 1.f : 0.f;
+                            const float hx = cc.x * ix[e], hy = cc.y * yi[e], hz = cc.z * zi[e];
+                            const float num = fmaf(fmaf(0.5f, gx, 0.5f), hx, fmaf(fmaf(0.5f, gy, 0.5f), hy, fmaf(fmaf(0.5f, gz, 0.5f), hz, qd[e])));
+                            const float den = fmaf(gx, cc.x, fmaf(gy, cc.y, fmaf(gz, cc.z, sig0)));
+                            const float c = __fdividef(num, den);
+                            pc[e] = c;
+                            ox[e] = gx * (2.f * c - ix[e]);
+                            oyr[e] = gy * (2.f * c - yi[e]);
+                            ozr[e] = gz * (2.f * c - zi[e]);
+                            any |= act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
+                        }
+                    }
+                    float hi[N], lo[N];
+#pragma unroll
+                    for (int e = 0; e < N; ++e) {
+                        const int r = C0 + e;
+                        if (act) {
+                            px[r] = ox[e]; oy[r] = oyr[e]; oz[r] = ozr[e];
+                            if (store_y) __stcg(fy_st + r * DOS_TK, oyr[e]);
+                            if (store_z) __stcg(fz_st + r * DOS_TJ, ozr[e]);
+                        }
+                        tf32_split(act ? pc[e] : 0.f, hi[e], lo[e]);
+                    }
+                    if constexpr (C0 == 0) {
+                        TRACE(4);
+                        wait_bar(&psi_empty[gs % PSL], ((gs / PSL) & 1) ^ 1, &s_abort, p.abort_flag, 32);
+                        tc_fence_after();
+                        TRACE(5);
+                    }
+                    tmem_st_n<N>(tp + C0, hi);
+                    tmem_st_n<N>(tp + A8 + C0, lo);
+                };
+                [&]<int... I>(std::integer_sequence<int, I...>) { (chunk.template operator()<I * CH>(), ...); }(
+                    std::make_integer_sequence<int, (AG + CH - 1) / CH>{});
+                fy_st += fy_inc; fz_st += fz_inc;
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();                         // also orders every lane's face stores before the progress word
                 if (lane == 0) {
+                    mbar_arrive(&q_empty[gs % DQS]);
                     mbar_arrive(&psi_full[gs % PSL]);
                     st_release_cta(&s_prog[warp], t + 1);
                 }
+                TRACE(6);
             }
             gs0 += T;
             if (has_y || has_z) fs0 += T;
@@ -581,7 +716,7 @@ static const UShape *umma_shape(int per_oct)
     static const UShape shapes[] = {
         {1, 1, sweep_umma_kernel<1, 1>}, {3, 1, sweep_umma_kernel<3, 1>}, {6, 1, sweep_umma_kernel<6, 1>},
         {5, 2, sweep_umma_kernel<5, 2>}, {5, 3, sweep_umma_kernel<5, 3>}, {7, 3, sweep_umma_kernel<7, 3>},
-        {7, 4, sweep_umma_kernel<7, 4>}, {9, 4, sweep_umma_kernel<9, 4>},
+        {7, 4, sweep_umma_kernel<7, 4>}, {12, 3, sweep_umma_kernel<12, 3>},
     };
     for (const UShape &s : shapes)
         if (s.ag * s.ng == per_oct) return &s;
@@ -613,6 +748,13 @@ cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int 
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if (s->ng >= 3) {
+        // the register re-allocation inside the kernel must fit the CTA's allocation at launch (else it would block)
+        cudaFuncAttributes fa;
+        if ((e = cudaFuncGetAttributes(&fa, s->fn)) != cudaSuccess) return e;
+        const int threads = (4 * s->ng + 12) * 32;
+        if (fa.numRegs * threads < (umma_reg_compute(s->ng) * 4 * s->ng + umma_reg_helper(s->ng) * 12) * 32) return cudaErrorLaunchOutOfResources;
+    }
     // one CTA per SM: each allocates all 512 tensor-memory columns
     *grid_out = sms < n_items ? sms : n_items;
     return cudaSuccess;
