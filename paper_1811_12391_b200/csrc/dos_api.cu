@@ -158,12 +158,13 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
     return DOS_OK;
 }
 
-// Choice and shape of the sweep for the current option values. The tensor-memory sweep (dos_sweep_umma.cu) is the
-// default wherever the quadrature admits it; the FFMA sweep is the fallback and the A/B partner.
+// Choice and shape of the sweep for the current option values. Default: the tensor-memory sweep (dos_sweep_umma.cu) from
+// P4 up (28 / 36 moments per cell: the two contractions are 70-80 % of the arithmetic) wherever the quadrature admits
+// it, the FFMA sweep below (measured: S8/P3 on 256x256x64 2.9 ms per sweep against 3.7) and as the fallback.
 static cudaError_t configure_sweep(dos_ctx *c)
 {
     const bool ffma_ok = dos_sweep_ffma_angles_per_warp(c->per_oct, c->L, 0) != 0;
-    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok) || !ffma_ok;
+    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok && c->MP >= 28) || !ffma_ok;
     if (want_umma) {
         if (!c->umma_ok) return cudaErrorInvalidValue;
         int grid = 0;

@@ -13,14 +13,19 @@
 //               x_local = step - (jj + kk): the KBA wavefront inside the warp, as in dos_sweep_ffma.cu.
 //   M2D         D_q[row][angle] = sum_lm A[row][lm] B[lm][angle], A = the row's source moments with the octant's
 //               mirror signs applied (Y_lm of a mirrored direction is +-Y_lm: the sign depends on (l,m) and the mirror
-//               only), split into TF32 hi + lo by the `split` warps and written to shared memory in the UMMA K-major
-//               core-matrix layout; B = (2l+1) Y_lm of octant 0's angles, pre-split on the host. 3 terms
-//               (lo*hi, hi*lo, hi*hi) x K/8 instructions, issued by one thread, accumulator ring in TMEM.
+//               only), split into TF32 hi + lo and written to shared memory in the UMMA K-major core-matrix layout;
+//               B = (2l+1) Y_lm of octant 0's angles, pre-split on the host. 3 terms (lo*hi, hi*lo, hi*hi) x K/8
+//               instructions, issued by one thread, accumulator ring in TMEM.
 //   cell update compute warp (octant q, angle group g) reads its AG columns of D_q straight from TMEM (tcgen05.ld),
 //               takes the y/z inflow from the neighbouring lanes by shuffle (or from the staged tile-inflow faces),
 //               and writes psi_c, split into hi + lo, back to TMEM (tcgen05.st) as the A operand of
-//   D2M         D_phi[row][lm] = sum_a psi[row][a] w_a Y_lm(a) (A from TMEM, B from shared memory), after which the
-//               `epilogue` warps read D_phi (tcgen05.ld), apply the mirror signs and red.global.add.v4 into phi.
+//   D2M         D_phi[row][lm] = sum_a psi[row][a] w_a Y_lm(a) (A from TMEM, B from shared memory); D_phi is read back
+//               (tcgen05.ld), given the mirror signs and added to phi with red.global.add.v4.
+//   one warp kind  the NG compute warps of an octant also share the staging (cp.async of their 16-byte pieces of every
+//               row, LA steps ahead), the split (SA steps ahead) and the read-back of D_phi (EB steps behind): lane =
+//               row in all four jobs. Measured: with separate staging / read-back warps only 12 of 24 warps carried
+//               cell updates, each a long dependent chain, and the SM sat at 0.2-0.4 IPC per scheduler; with every warp
+//               a compute warp there are twice as many chains in flight and half as many angles per chain.
 //   tile faces  as in dos_sweep_ffma.cu: outflow of the tile's last j / k lanes goes to an L2-resident buffer indexed
 //               by wavefront diagonal, published every `chunk` steps by the service warp (st.release.gpu), acquired by
 //               the downwind CTA's service warp, staged by its feeder warp with bulk copies.
@@ -35,7 +40,9 @@ namespace {
 using namespace sm100;
 
 constexpr int RAW = 4;       // ring of staged source-moment rows (steps)
-constexpr int LA = 3;        // steps between issuing a row's bulk copy and using it
+constexpr int LA = 4;        // steps between issuing a row's cp.async and the cell update that uses it
+constexpr int SA = 2;        // steps the TF32 split (and with it the M2D) runs ahead of the cell update
+constexpr int EB = 2;        // steps the read-back of D_phi lags behind the cell update
 constexpr int ASL = 2;       // ring of split A operands (hi, lo) in shared memory
 constexpr int DQS = 4;       // ring of M2D accumulators in TMEM
 constexpr int PSL = 2;       // ring of psi operands (hi, lo) in TMEM
@@ -96,25 +103,6 @@ __device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_
     atomicExch(g_abort, 1);
 }
 
-// Slow path of the cell update: at least one extrapolated outflow was negative. Faces found negative are pinned to
-// zero together, the balance is re-solved, and the pinned set only grows (R12).
-__device__ __forceinline__ void dd_fixup(float &pc, float &ox, float &oy, float &oz, float q, float st, float cx, float cy, float cz,
-                                         float ix, float iy, float iz)
-{
-    const float hx = cx * ix, hy = cy * iy, hz = cz * iz;
-    bool fx = false, fy = false, fz = false;
-#pragma unroll 1
-    do {
-        fx |= ox < 0.f; fy |= oy < 0.f; fz |= oz < 0.f;
-        const float num = q + (fx ? 0.5f * hx : hx) + (fy ? 0.5f * hy : hy) + (fz ? 0.5f * hz : hz);
-        const float den = st + (fx ? 0.f : cx) + (fy ? 0.f : cy) + (fz ? 0.f : cz);
-        pc = __fdividef(num, den);
-        ox = fx ? 0.f : 2.f * pc - ix;
-        oy = fy ? 0.f : 2.f * pc - iy;
-        oz = fz ? 0.f : 2.f * pc - iz;
-    } while (fminf(ox, fminf(oy, oz)) < 0.f);
-}
-
 // hi = x rounded to TF32 (round half away from zero on the bit pattern; inputs are finite), lo = x - hi (exact in
 // fp32; the tensor core reads its leading 11 bits: an error <= 2^-22 |x|)
 __device__ __forceinline__ void tf32_split(float x, float &hi, float &lo)
@@ -122,9 +110,6 @@ __device__ __forceinline__ void tf32_split(float x, float &hi, float &lo)
     hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
     lo = x - hi;
 }
-
-__host__ __device__ constexpr int umma_reg_compute(int ng) { return ng == 4 ? 96 : 120; }
-__host__ __device__ constexpr int umma_reg_helper(int) { return 40; }
 
 struct Geom {          // one octant's (j,k) column of this lane
     bool valid;
@@ -146,66 +131,26 @@ __device__ __forceinline__ Geom make_geom(const SweepUArgs &p, int o, int tj, in
     return g;
 }
 
-// Epilogue of one row: D_phi columns [C0, MP) -> mirror signs -> phi[cell][C0..MP) by red.global.add.v4, 8 columns at a time.
-template <int MP, int C0>
-__device__ __forceinline__ void epilogue_row(unsigned taddr, const unsigned *sgn, float *phi, bool on)
+// One 16-byte piece (4 moments) of a row: mirror signs, TF32 hi / lo, into the UMMA core-matrix layout.
+__device__ __forceinline__ void split_piece(const float4 *src, const unsigned *sgn, float4 *dh, float4 *dl, bool on)
 {
-    if constexpr (C0 < MP) {
-        constexpr int N = MP - C0 < 8 ? MP - C0 : 8;
-        float v[N];
-        tmem_ld_n<N>(taddr + C0, v);
-        tmem_wait_ld();
-        if (on && !(DOS_UMMA_ABL & 2)) {
-#pragma unroll
-            for (int e = 0; e < N; e += 4) {
-                const uint4 s = *reinterpret_cast<const uint4 *>(sgn + C0 + e);
-                red_add_v4(phi + C0 + e, __uint_as_float(__float_as_uint(v[e]) ^ s.x), __uint_as_float(__float_as_uint(v[e + 1]) ^ s.y),
-                           __uint_as_float(__float_as_uint(v[e + 2]) ^ s.z), __uint_as_float(__float_as_uint(v[e + 3]) ^ s.w));
-            }
-        }
-        epilogue_row<MP, C0 + N>(taddr, sgn, phi, on);
-    }
-}
-
-// Split warp, one row of NQ float4: stage (cp.async) and convert (mirror signs, TF32 hi / lo, UMMA core-matrix layout).
-template <int NQ>
-__device__ __forceinline__ void split_issue(float *dst, const float *src)
-{
-#pragma unroll
-    for (int c = 0; c < NQ; ++c) cp_async16(dst + 4 * c, src + 4 * c);
-}
-template <int NQ>
-__device__ __forceinline__ void split_row(const float4 *src, const unsigned *sgn, float4 *dh, float4 *dl, bool on)
-{
-#pragma unroll
-    for (int b = 0; b < NQ; b += 3) {                 // 3 float4 in flight: the helper warps live in 40 registers
-        float4 x[3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-            if (b + c < NQ) x[c] = on ? src[b + c] : make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-            if (b + c < NQ) {
-                const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn + 4 * (b + c));
-                float4 h, l;
-                tf32_split(__uint_as_float(__float_as_uint(x[c].x) ^ s4.x), h.x, l.x);
-                tf32_split(__uint_as_float(__float_as_uint(x[c].y) ^ s4.y), h.y, l.y);
-                tf32_split(__uint_as_float(__float_as_uint(x[c].z) ^ s4.z), h.z, l.z);
-                tf32_split(__uint_as_float(__float_as_uint(x[c].w) ^ s4.w), h.w, l.w);
-                dh[(b + c) * 8] = h;
-                dl[(b + c) * 8] = l;
-            }
-    }
+    const float4 x = on ? *src : make_float4(0.f, 0.f, 0.f, 0.f);
+    const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn);
+    float4 h, l;
+    tf32_split(__uint_as_float(__float_as_uint(x.x) ^ s4.x), h.x, l.x);
+    tf32_split(__uint_as_float(__float_as_uint(x.y) ^ s4.y), h.y, l.y);
+    tf32_split(__uint_as_float(__float_as_uint(x.z) ^ s4.z), h.z, l.z);
+    tf32_split(__uint_as_float(__float_as_uint(x.w) ^ s4.w), h.w, l.w);
+    *dh = h;
+    *dl = l;
 }
 
 // Warp roles (NG compute warps per octant, AG angles each):
-//   [0, 4 NG)            compute: octant q = warp % 4, angle group g = warp / 4
-//   [4 NG, 4 NG + 4)     split:   octant q; bulk copies of the rows' source moments, mirror signs, TF32 split
-//   [.. + 4, .. + 8)     epilogue: octant q; D_phi -> phi
-//   .. + 8               M2D issuer (one elected lane)      .. + 9   D2M issuer
-//   .. + 10              feeder (tile-inflow faces)         .. + 11  service (global hand-off flags)
+//   [0, 4 NG)   compute: octant q = warp % 4, angle group g = warp / 4 (also: its share of staging, split, read-back)
+//   4 NG        M2D issuer (one elected lane)      4 NG + 1   D2M issuer
+//   4 NG + 2    feeder (tile-inflow faces)         4 NG + 3   service (global hand-off flags)
 template <int AG, int NG>
-__global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const SweepUArgs p)
+__global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const SweepUArgs p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int A = p.per_oct, MP = p.MP, KP = (MP + 7) & ~7, NCH = KP / 4, A8 = (A + 7) & ~7, NAP = (A + 15) & ~15, NMP = (MP + 15) & ~15;
@@ -225,7 +170,7 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
     unsigned *s_sign = reinterpret_cast<unsigned *>(carve((size_t)8 * MP * 4));                 // [8 octants][MP] 0 or 0x80000000
     uint64_t *bars = reinterpret_cast<uint64_t *>(carve(64 * 8));
     int *s_prog = reinterpret_cast<int *>(carve(32 * 4));                                       // [NCW] steps finished per compute warp
-    uint64_t *raw_full = bars;            // [RAW][4]
+    uint64_t *raw_full = bars;            // [RAW][4 octants]
     uint64_t *a_full = bars + 16;         // [ASL]
     uint64_t *a_empty = bars + 18;
     uint64_t *q_full = bars + 20;         // [DQS]
@@ -239,8 +184,7 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
     __shared__ unsigned s_tmem;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, q = warp & 3;
-    const bool is_compute = warp < NCW, is_split = warp >= NCW && warp < NCW + 4, is_epi = warp >= NCW + 4 && warp < NCW + 8;
-    const bool is_m2d = warp == NCW + 8, is_d2m = warp == NCW + 9, is_feed = warp == NCW + 10, is_service = warp == NCW + 11;
+    const bool is_m2d = warp == NCW, is_d2m = warp == NCW + 1, is_feed = warp == NCW + 2, is_service = warp == NCW + 3;
     const int nx = p.nx, T = nx + DOS_SKEW;
     const size_t fstride_y = (size_t)(nx + DOS_FACE_PAD) * A * DOS_TK, fstride_z = (size_t)(nx + DOS_FACE_PAD) * A * DOS_TJ;
 
@@ -253,11 +197,11 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
     for (int i = tid; i < p.n_mat; i += blockDim.x) s_sig[i] = p.sig_t[i];
     for (int i = tid; i < 8 * MP; i += blockDim.x) s_sign[i] = p.signs[i];
     if (tid == 0) {
-        for (int i = 0; i < 16; ++i) mbar_init(&raw_full[i], 32);
-        for (int i = 0; i < ASL; ++i) { mbar_init(&a_full[i], 4); mbar_init(&a_empty[i], 1); }
+        for (int i = 0; i < 16; ++i) mbar_init(&raw_full[i], 32 * NG);      // one cp.async arrival per thread of the octant's warps
+        for (int i = 0; i < ASL; ++i) { mbar_init(&a_full[i], NCW); mbar_init(&a_empty[i], 1); }
         for (int i = 0; i < DQS; ++i) { mbar_init(&q_full[i], 1); mbar_init(&q_empty[i], NCW); }
         for (int i = 0; i < PSL; ++i) { mbar_init(&psi_full[i], NCW); mbar_init(&psi_empty[i], 1); }
-        for (int i = 0; i < DPS; ++i) { mbar_init(&phi_full[i], 1); mbar_init(&phi_empty[i], 4); }
+        for (int i = 0; i < DPS; ++i) { mbar_init(&phi_full[i], 1); mbar_init(&phi_empty[i], NCW); }
         for (int i = 0; i < RFU; ++i) mbar_init(&fin_full[i], 1);
         s_abort = 0;
         mbar_init_fence();
@@ -271,11 +215,10 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
     // TMEM columns: [0, DQS*NAP) M2D accumulators | psi operands [PSL][hi A8 | lo A8] | [DPS][NMP] D2M accumulators
     const unsigned tm_dq = tm, tm_psi = tm + DQS * NAP, tm_dphi = tm_psi + PSL * 2 * A8;
     const unsigned lane_base = (unsigned)(q * 32) << 16;
-    if (is_compute) {
+    if (warp < 4) {
         // the K padding columns of the psi operands must be finite (they meet zero rows of B): zero them once
         float z[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        if (warp < 4)
-            for (int c = 0; c < PSL * 2 * A8; c += 8) tmem_st<8>(tm_psi + lane_base + c, z);
+        for (int c = 0; c < PSL * 2 * A8; c += 8) tmem_st<8>(tm_psi + lane_base + c, z);
         tmem_wait_st();
     }
     tc_fence_before();
@@ -284,14 +227,13 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
 
     unsigned gs0 = 0;      // global step counter at the start of the current item (ring slots and phases follow it)
     unsigned fs0 = 0;      // the same for the tile-inflow ring, which only items with an upwind tile use
-    // Every role runs its own loop over the work items (so that each role's code lies behind its own setmaxnreg and
-    // ptxas can give it its own register budget); all of them meet in the two barriers of next_item().
     int quad = 0, tj = 0, tk = 0, fid = 0;
     bool has_y = false, has_z = false;
 #if DOS_UMMA_TRACE
     bool trace_on = false;
     long long *trace_buf = reinterpret_cast<long long *>(p.fz);      // measurement build: the z-face buffer of item 0 is sacrificed
 #endif
+    // every role runs its own loop over the work items; all of them meet in the two barriers of next_item()
     auto next_item = [&]() -> bool {
         __syncthreads();                              // every role has drained the previous item
         if (tid == 0) s_item = atomicAdd(p.queue, 1);
@@ -308,16 +250,8 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
 #endif
         return true;
     };
-    // Register re-allocation (warp roles come in aligned groups of 4 warps, as setmaxnreg requires): the compute warps
-    // carry 3 face fluxes per angle plus the cell update's temporaries, the helper warps need little.
-    // setmaxnreg re-divides the CTA's OWN register allocation (threads x registers at launch), it cannot draw on the
-    // rest of the register file: with more than the launch total the increase blocks for ever. NG = 4: 896 threads x 72 =
-    // 16 warps x 96 + 12 x 40; NG = 3: 768 x 80 = 12 x 120 + 12 x 40 (dos_sweep_umma_grid checks the launch count).
-    constexpr int REG_C = umma_reg_compute(NG), REG_H = umma_reg_helper(NG);
-    constexpr bool REALLOC = NG >= 3;
 
     if (is_service) {
-        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
         while (next_item()) {
             // ------- service warp: publishes this item's progress, follows the two upwind items' progress -------
             const int *up_y = p.done + (has_y ? fid - 1 : fid), *up_z = p.done + (has_z ? fid - p.ntj : fid);
@@ -354,13 +288,12 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                         __nanosleep(DOS_POLL_NS);
                     }
                 } else {
-                    __nanosleep(2 * DOS_POLL_NS);
+                    __nanosleep(4 * DOS_POLL_NS);
                 }
             }
             gs0 += T;
         }
     } else if (is_feed) {
-        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
         while (next_item()) {
             // ------- feeder warp: bulk copies of the tile-inflow faces the upwind tiles have published -------
             // step s of octant qq needs fy_in[s][A][TK] and fz_in[s][A][TJ]: two contiguous blocks per octant.
@@ -384,7 +317,7 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                         for (int d = 16; d >= 1; d >>= 1) mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, d));
                         if (mn >= s - RFU + 1) break;
                         if (((++spins) & 255) == 0 && *(volatile int *)&s_abort) break;
-                        __nanosleep(32);
+                        __nanosleep(100);
                     }
                     while (allowed_c < s) {           // wait until the upwind tiles have published step s
                         allowed_c = ld_acquire_cta(&s_allowed);
@@ -401,7 +334,6 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             gs0 += T;
         }
     } else if (is_m2d) {
-        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
         while (next_item()) {
             // ------- M2D issuer: D_q[slot] = A_lo B_hi + A_hi B_lo + A_hi B_hi -------
             __syncthreads();                          // S2
@@ -413,9 +345,9 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
                 TRACE(0);
-                wait_bar(&a_full[gs % ASL], (gs / ASL) & 1, &s_abort, p.abort_flag);
+                wait_bar(&a_full[gs % ASL], (gs / ASL) & 1, &s_abort, p.abort_flag, 100);
                 TRACE(1);
-                wait_bar(&q_empty[gs % DQS], ((gs / DQS) & 1) ^ 1, &s_abort, p.abort_flag);
+                wait_bar(&q_empty[gs % DQS], ((gs / DQS) & 1) ^ 1, &s_abort, p.abort_flag, 100);
                 TRACE(2);
                 tc_fence_after();
                 {
@@ -436,7 +368,6 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             gs0 += T;
         }
     } else if (is_d2m) {
-        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
         while (next_item()) {
             // ------- D2M issuer: D_phi[slot] = psi_lo B_hi + psi_hi B_lo + psi_hi B_hi (A operand in TMEM) -------
             __syncthreads();                          // S2
@@ -448,9 +379,9 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
                 TRACE(0);
-                wait_bar(&psi_full[gs % PSL], (gs / PSL) & 1, &s_abort, p.abort_flag);
+                wait_bar(&psi_full[gs % PSL], (gs / PSL) & 1, &s_abort, p.abort_flag, 100);
                 TRACE(1);
-                wait_bar(&phi_empty[gs % DPS], ((gs / DPS) & 1) ^ 1, &s_abort, p.abort_flag);
+                wait_bar(&phi_empty[gs % DPS], ((gs / DPS) & 1) ^ 1, &s_abort, p.abort_flag, 100);
                 TRACE(2);
                 tc_fence_after();
                 {
@@ -469,107 +400,12 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             }
             gs0 += T;
         }
-    } else if (is_split) {
-        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
+    } else {
+        // ---------------- compute warps ----------------
         while (next_item()) {
-            // this warp owns octant o = 4 quad + q; the lane owns one (j,k) column of its tile
-            const int o = quad * 4 + q;
+            const int o = quad * 4 + q;               // this warp's octant; the lane owns one (j,k) column of its tile
             const Geom g = make_geom(p, o, tj, tk, lane);
             const int row = q * 32 + lane;
-            // ------- split warp: bulk copy of each row's MP source moments, mirror signs, TF32 hi / lo, UMMA layout -------
-            __syncthreads();                          // S2
-            const float *qsrc = p.Q + g.cbase * MP;
-            const long long qinc = (long long)g.istep * MP;
-            const unsigned *sgn = s_sign + o * MP;
-            const int nq = MP / 4;
-            auto issue = [&](int s) {
-                // one 16-byte cp.async per 4 moments of this lane's row; the lane's arrival on the ring slot's mbarrier
-                // fires when they have landed
-                const bool on = (unsigned)(s - g.t_lo) < (unsigned)nx;
-                uint64_t *bar = &raw_full[((gs0 + s) % RAW) * 4 + q];
-                if (on && !(DOS_UMMA_ABL & 1)) {
-                    float *dst = s_raw + ((size_t)((gs0 + s) % RAW) * 128 + row) * MP;
-                    const float *src = qsrc + qinc * s;
-                    switch (nq) {
-                        case 1: split_issue<1>(dst, src); break;
-                        case 3: split_issue<3>(dst, src); break;
-                        case 4: split_issue<4>(dst, src); break;
-                        case 7: split_issue<7>(dst, src); break;
-                        default: split_issue<9>(dst, src); break;
-                    }
-                }
-                cp_async_mbar_arrive(bar);
-            };
-            for (int s = 0; s < LA && s < T; ++s) issue(s);
-#pragma unroll 1
-            for (int t = 0; t < T; ++t) {
-                const unsigned gs = gs0 + t;
-                TRACE(0);
-                if (t + LA < T) issue(t + LA);
-                TRACE(1);
-                wait_bar(&raw_full[(gs % RAW) * 4 + q], (gs / RAW) & 1, &s_abort, p.abort_flag);
-                TRACE(2);
-                wait_bar(&a_empty[gs % ASL], ((gs / ASL) & 1) ^ 1, &s_abort, p.abort_flag);
-                TRACE(3);
-                const bool on = (unsigned)(t - g.t_lo) < (unsigned)nx;
-                const float4 *src = reinterpret_cast<const float4 *>(s_raw + ((size_t)(gs % RAW) * 128 + row) * MP);
-                // element (row, chunk c): ((row / 8) * NCH + c) * 32 + (row % 8) * 4 floats
-                float4 *dh = reinterpret_cast<float4 *>(s_a + (size_t)(gs % ASL) * (2 * 16 * NCH * 32) + ((row >> 3) * NCH) * 32 + (row & 7) * 4);
-                float4 *dl = dh + 16 * NCH * 8;
-                switch (nq) {
-                    case 1: split_row<1>(src, sgn, dh, dl, on); break;
-                    case 3: split_row<3>(src, sgn, dh, dl, on); break;
-                    case 4: split_row<4>(src, sgn, dh, dl, on); break;
-                    case 7: split_row<7>(src, sgn, dh, dl, on); break;
-                    default: split_row<9>(src, sgn, dh, dl, on); break;
-                }
-                fence_proxy_async_smem();             // the stores above -> the UMMA's operand reads; the row reads -> the next bulk copy
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&a_full[gs % ASL]);
-                TRACE(4);
-            }
-            gs0 += T;
-        }
-    } else if (is_epi) {
-        if constexpr (REALLOC) setmaxnreg_dec<REG_H>();
-        while (next_item()) {
-            const int o = quad * 4 + q;
-            const Geom g = make_geom(p, o, tj, tk, lane);
-            // ------- epilogue warp: D_phi row -> mirror signs -> red.global.add into phi[cell][MP] -------
-            __syncthreads();                          // S2
-            float *phi_p = p.phi + g.cbase * MP;
-            const long long pinc = (long long)g.istep * MP;
-            const unsigned *sgn = s_sign + o * MP;
-#pragma unroll 1
-            for (int t = 0; t < T; ++t) {
-                const unsigned gs = gs0 + t;
-                TRACE(0);
-                wait_bar(&phi_full[gs % DPS], (gs / DPS) & 1, &s_abort, p.abort_flag);
-                TRACE(1);
-                tc_fence_after();
-                const bool on = (unsigned)(t - g.t_lo) < (unsigned)nx;
-                const unsigned ta = tm_dphi + lane_base + (gs % DPS) * NMP;
-                switch (MP) {
-                    case 4: epilogue_row<4, 0>(ta, sgn, phi_p, on); break;
-                    case 12: epilogue_row<12, 0>(ta, sgn, phi_p, on); break;
-                    case 16: epilogue_row<16, 0>(ta, sgn, phi_p, on); break;
-                    case 28: epilogue_row<28, 0>(ta, sgn, phi_p, on); break;
-                    default: epilogue_row<36, 0>(ta, sgn, phi_p, on); break;
-                }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&phi_empty[gs % DPS]);
-                TRACE(2);
-                phi_p += pinc;
-            }
-            gs0 += T;
-        }
-    } else {
-        // ---------------- compute warps: diamond difference, face hand-off ----------------
-        if constexpr (REALLOC) setmaxnreg_inc<REG_C>();
-        while (next_item()) {
-            const int o = quad * 4 + q;
-            const Geom g = make_geom(p, o, tj, tk, lane);
             const int grp = warp >> 2, a0 = grp * AG;
             const int jj = lane & (DOS_TJ - 1), kk = lane / DOS_TJ;
             const bool in_y = jj == 0, in_z = kk == 0;
@@ -582,13 +418,71 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
             const float *finy = s_finy + (q * A + a0) * DOS_TK + kk, *finz = s_finz + (q * A + a0) * DOS_TJ + jj;
             const uint8_t *mat_p = p.mat + g.cbase;
             const int istep = g.istep, t_lo = g.t_lo;
+            const long long cinc = (long long)istep * MP;                // floats between this lane's consecutive cells
+            const float *qsrc = p.Q + g.cbase * MP;
+            float *phi_base = p.phi + g.cbase * MP;
+            const unsigned *sgn = s_sign + o * MP;
+            const int nq = MP / 4;                                       // 16-byte pieces of a row; this warp takes grp, grp + NG, ...
             __syncthreads();                          // S2
             const float4 *cdd4 = reinterpret_cast<const float4 *>(s_cdd) + a0;     // (cx, cy, cz, cx+cy+cz) per angle: warp-uniform reads
+
+            // staging: this lane's pieces of its row of step s, by cp.async; the thread's arrival on the ring slot's
+            // mbarrier fires when they have landed
+            auto stage = [&](int s) {
+                const bool on = (unsigned)(s - t_lo) < (unsigned)nx;
+                const unsigned gsx = gs0 + s;
+                if (on && !(DOS_UMMA_ABL & 1)) {
+                    float *dst = s_raw + ((size_t)(gsx % RAW) * 128 + row) * MP;
+                    const float *src = qsrc + cinc * s;
+                    for (int c = grp; c < nq; c += NG) cp_async16(dst + 4 * c, src + 4 * c);
+                }
+                cp_async_mbar_arrive(&raw_full[(gsx % RAW) * 4 + q]);
+            };
+            // split: this lane's pieces of its row of step s -> mirror signs, TF32 hi / lo, UMMA layout -> a_full
+            auto split = [&](int s) {
+                const unsigned gsx = gs0 + s;
+                wait_bar(&raw_full[(gsx % RAW) * 4 + q], (gsx / RAW) & 1, &s_abort, p.abort_flag, 32);
+                wait_bar(&a_empty[gsx % ASL], ((gsx / ASL) & 1) ^ 1, &s_abort, p.abort_flag, 32);
+                const bool on = (unsigned)(s - t_lo) < (unsigned)nx;
+                const float4 *src = reinterpret_cast<const float4 *>(s_raw + ((size_t)(gsx % RAW) * 128 + row) * MP);
+                // element (row, piece c): ((row / 8) * NCH + c) * 32 + (row % 8) * 4 floats
+                float4 *dh = reinterpret_cast<float4 *>(s_a + (size_t)(gsx % ASL) * (2 * 16 * NCH * 32) + ((row >> 3) * NCH) * 32 + (row & 7) * 4);
+                float4 *dl = dh + 16 * NCH * 8;
+                for (int c = grp; c < nq; c += NG) split_piece(src + c, sgn + 4 * c, dh + c * 8, dl + c * 8, on);
+                fence_proxy_async_smem();             // the stores above -> the UMMA's operand reads
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&a_full[gsx % ASL]);
+            };
+            // read-back: this warp's 4-column groups of D_phi of step s -> mirror signs -> red.global.add.v4 into phi
+            auto readback = [&](int s) {
+                const unsigned gsx = gs0 + s;
+                wait_bar(&phi_full[gsx % DPS], (gsx / DPS) & 1, &s_abort, p.abort_flag, 32);
+                tc_fence_after();
+                const bool on = (unsigned)(s - t_lo) < (unsigned)nx;
+                const unsigned ta = tm_dphi + lane_base + (gsx % DPS) * NMP;
+                float *phi_p = phi_base + cinc * s;
+                for (int c = grp; c < nq; c += NG) {
+                    float v[4];
+                    tmem_ld<4>(ta + 4 * c, v);
+                    tmem_wait_ld();
+                    if (on && !(DOS_UMMA_ABL & 2)) {
+                        const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn + 4 * c);
+                        red_add_v4(phi_p + 4 * c, __uint_as_float(__float_as_uint(v[0]) ^ s4.x), __uint_as_float(__float_as_uint(v[1]) ^ s4.y),
+                                   __uint_as_float(__float_as_uint(v[2]) ^ s4.z), __uint_as_float(__float_as_uint(v[3]) ^ s4.w));
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&phi_empty[gsx % DPS]);
+            };
+
             float px[AG], oy[AG], oz[AG];
 #pragma unroll
             for (int r = 0; r < AG; ++r) px[r] = oy[r] = oz[r] = 0.f;
             auto mat_of = [&](int s) -> int { return ((unsigned)(s - t_lo) < (unsigned)nx) ? min((int)__ldg(mat_p + (long long)istep * s), p.n_mat - 1) : 0; };
             int m_cur = mat_of(0), m_nxt = mat_of(1);
+            for (int s = 0; s < LA && s < T; ++s) stage(s);
+            for (int s = 0; s < SA && s < T; ++s) split(s);
 
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
@@ -598,12 +492,13 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                 m_cur = m_nxt;
                 m_nxt = mat_of(t + 2);
                 TRACE(0);
+                if (t + LA < T) stage(t + LA);
                 wait_bar(&q_full[gs % DQS], (gs / DQS) & 1, &s_abort, p.abort_flag, 32);
                 TRACE(1);
                 tc_fence_after();
                 const unsigned fs = fs0 + t;
                 if (has_y || has_z) wait_bar(&fin_full[fs % RFU], (fs / RFU) & 1, &s_abort, p.abort_flag, 32);
-                TRACE(3);
+                TRACE(2);
                 const int fslot = (int)(fs % RFU) * 4 * A;
                 const float *rden = s_rden + m0 * A + a0;
                 const float sig0 = s_sig[m0];
@@ -616,9 +511,9 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                 // pinned face has outflow exactly 0, so "pinned" is read off the outflow itself (o <= 0): a face whose
                 // unpinned outflow is exactly 0 may be treated as pinned, because pinning any other face lowers psi_c and
                 // would pin it in the next pass anyway. A pass with nothing new to pin reproduces its input.
-                // Each chunk reads its CH columns of the discrete source from tensor memory and writes its psi_c (TF32
+                // Each chunk reads its columns of the discrete source from tensor memory and writes its psi_c (TF32
                 // hi + lo) back as the D2M's A operand, so no per-angle array outlives a chunk except the 3 face fluxes.
-                constexpr int CH = (AG % 4 == 0 || AG == 7) ? 4 : (AG >= 3 ? 3 : AG);
+                constexpr int CH = AG <= 4 ? AG : (AG % 3 == 0 ? 3 : 4);
                 auto chunk = [&]<int C0>() {
                     constexpr int N = AG - C0 < CH ? AG - C0 : CH;
                     float qd[N], ix[N], yi[N], zi[N], ox[N], oyr[N], ozr[N], pc[N];
@@ -670,10 +565,10 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                         tf32_split(act ? pc[e] : 0.f, hi[e], lo[e]);
                     }
                     if constexpr (C0 == 0) {
-                        TRACE(4);
+                        TRACE(3);
                         wait_bar(&psi_empty[gs % PSL], ((gs / PSL) & 1) ^ 1, &s_abort, p.abort_flag, 32);
                         tc_fence_after();
-                        TRACE(5);
+                        TRACE(4);
                     }
                     tmem_st_n<N>(tp + C0, hi);
                     tmem_st_n<N>(tp + A8 + C0, lo);
@@ -689,8 +584,13 @@ __global__ void __launch_bounds__((4 * NG + 12) * 32, 1) sweep_umma_kernel(const
                     mbar_arrive(&psi_full[gs % PSL]);
                     st_release_cta(&s_prog[warp], t + 1);
                 }
+                TRACE(5);
+                if (t + SA < T) split(t + SA);
                 TRACE(6);
+                if (t >= EB) readback(t - EB);
+                TRACE(7);
             }
+            for (int s = T - EB > 0 ? T - EB : 0; s < T; ++s) readback(s);
             gs0 += T;
             if (has_y || has_z) fs0 += T;
         }
@@ -712,11 +612,14 @@ struct UShape { int ag, ng; sweep_u_fn fn; };
 static const UShape *umma_shape(int per_oct)
 {
     // (angles per compute warp, compute warps per octant) for the level-symmetric sets: S2 1, S4 3, S6 6, S8 10,
-    // S10 15, S12 21, S14 28, S16 36 angles per octant
+    // S10 15, S12 21, S14 28, S16 36 angles per octant. Measured at S16/P5 on 256x256x64 (ms per sweep): 6 angles x 6
+    // warps 9.47, 9 x 4 8.11, 12 x 3 7.43, 18 x 2 8.18; at S8/P3: 2 x 5 3.71, 5 x 2 3.78, 10 x 1 4.94 -- every warp
+    // pays a fixed per-step cost (waits, arrivals, fences, its share of staging / split / read-back), so few warps with
+    // many angles win until the chains get too long.
     static const UShape shapes[] = {
-        {1, 1, sweep_umma_kernel<1, 1>}, {3, 1, sweep_umma_kernel<3, 1>}, {6, 1, sweep_umma_kernel<6, 1>},
-        {5, 2, sweep_umma_kernel<5, 2>}, {5, 3, sweep_umma_kernel<5, 3>}, {7, 3, sweep_umma_kernel<7, 3>},
-        {7, 4, sweep_umma_kernel<7, 4>}, {12, 3, sweep_umma_kernel<12, 3>},
+        {1, 1, sweep_umma_kernel<1, 1>}, {1, 3, sweep_umma_kernel<1, 3>}, {2, 3, sweep_umma_kernel<2, 3>},
+        {2, 5, sweep_umma_kernel<2, 5>}, {3, 5, sweep_umma_kernel<3, 5>}, {3, 7, sweep_umma_kernel<3, 7>},
+        {4, 7, sweep_umma_kernel<4, 7>}, {12, 3, sweep_umma_kernel<12, 3>},
     };
     for (const UShape &s : shapes)
         if (s.ag * s.ng == per_oct) return &s;
@@ -748,13 +651,6 @@ cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int 
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if (s->ng >= 3) {
-        // the register re-allocation inside the kernel must fit the CTA's allocation at launch (else it would block)
-        cudaFuncAttributes fa;
-        if ((e = cudaFuncGetAttributes(&fa, s->fn)) != cudaSuccess) return e;
-        const int threads = (4 * s->ng + 12) * 32;
-        if (fa.numRegs * threads < (umma_reg_compute(s->ng) * 4 * s->ng + umma_reg_helper(s->ng) * 12) * 32) return cudaErrorLaunchOutOfResources;
-    }
     // one CTA per SM: each allocates all 512 tensor-memory columns
     *grid_out = sms < n_items ? sms : n_items;
     return cudaSuccess;
@@ -765,6 +661,6 @@ cudaError_t dos_launch_sweep_umma(const SweepUArgs &a, int L, int grid, cudaStre
     const UShape *s = umma_shape(a.per_oct);
     if (!s) return cudaErrorInvalidValue;
     const size_t smem = umma_smem(dos_mpad(L), a.per_oct, a.n_mat);
-    s->fn<<<grid, (4 * s->ng + 12) * 32, smem, st>>>(a);
+    s->fn<<<grid, (4 * s->ng + 4) * 32, smem, st>>>(a);
     return cudaGetLastError();
 }
