@@ -12,15 +12,18 @@ cell-angle-group updates/s over the whole step; `ms_per_step` is the cone-beam d
              between steps, max over ranks
   e2e        the same step through the C ABI with HOST buffers: material grid copied in from pinned
              memory (dos_set_material_host), dose map copied out (dos_dose_host), wall clock
-  roofline   the sweep kernel: algorithmic flop per launch / its mean CUDA-event duration inside the
-             timed region, against the FP32 pipe peak (the sweep's arithmetic intensity is 4-13x the
-             ridge point); the same for algorithmic bytes against MEASURED_PEAKS.json's HBM copy
-             bandwidth under roofline.hbm
+  roofline   the sweep kernel: algorithmic (compulsory) bytes per launch, (12 M + 1) N_v (read
+             Q_fix[M] and phi_old[M], write phi_new[M], 1 B material id), / its mean CUDA-event duration inside
+             the timed region, against MEASURED_PEAKS.json's HBM copy bandwidth; `traffic` = measured DRAM bytes
+             per launch from the ncu capture kept under profiles/; the FP32-pipe view (algorithmic flop against
+             SMs x 128 lanes x 2 x clock) under roofline.alu
   cpu_baseline  the fp64 oracle, as it stands, on this box's host cores, on a bounded sample
 
 --impl reference times the oracle itself (there is no reference implementation: the paper's program is
-closed source). N > 1: one process per GPU (torchrun), independent replicas of the problem (config4:
-source positions sharded, dose maps all-reduced), no collective on the data path otherwise.
+closed source). N > 1: one process per GPU (under torchrun, or spawned by this script when WORLD_SIZE is
+unset): a single projection does not shard, so every rank runs an independent replica ("weak"); config4's
+36 source positions are sharded over the ranks (scan.shard_positions) and the partial dose maps summed with
+one all-reduce (scan.all_reduce_dose), the only exchange the method has ("strong").
 """
 from __future__ import annotations
 
@@ -45,6 +48,9 @@ WORKLOADS = {
     "config3": "config3: 128x128x64 water cylinder, G=19, S16 (288 angles), P5, 20 iterations, one projection",
     "config4": "config4: 256x256x64 abdomen-like phantom, G=19, S8, P3, 15 iterations, 36-position axial scan, doses summed",
     "config5": "config5: 256^3 abdomen-like phantom, G=19, S16 (288 angles), P5, 20 iterations, one projection",
+    # the shape of the paper's own runs (Tables 2 and 6); context, not a BASELINE config
+    "paper_coarse": "paper-shaped: 64x64x16 (7.81 mm), 35 cm water cylinder, 7 groups 10-100 keV, S6/P0 (or --sn/--pl), 20 iterations, 16-position scan (--positions 1 = single projection)",
+    "paper_fine": "paper-shaped: 256x256x64 (1.95 mm), 35 cm water cylinder, 7 groups 10-100 keV, S6/P0 (or --sn/--pl), 20 iterations, 16-position scan (--positions 1 = single projection)",
 }
 # bounded oracle samples (about 10-30 s of CPU work): same mesh/quadrature/P_L, fewer groups/iterations;
 # the work per cell-angle-group update is the same as in the full workload
@@ -54,6 +60,8 @@ ORACLE_SAMPLE = {
     "config3": (dict(n_group=1, n_iter=1), "config3 mesh/S16/P5, 1 group, 1 source iteration"),
     "config4": (dict(n_group=1, n_iter=1, n_pos=1), "config4 mesh/S8/P3, 1 position, 1 group, 1 source iteration"),
     "config5": (dict(nz=16, n_group=1, n_iter=1), "config5 in-plane mesh 256x256, S16/P5, 16 of 256 slices, 1 group, 1 iteration"),
+    "paper_coarse": (dict(n_pos=1), "paper_coarse, one source position in full (7 groups x 20 iterations)"),
+    "paper_fine": (dict(n_pos=1, n_iter=1), "paper_fine, one source position, 7 groups x 1 source iteration"),
 }
 
 
@@ -115,8 +123,18 @@ class ClockSampler:
 
 
 def _cores():
+    """Threads the oracle uses: OMP_NUM_THREADS if set, else the PHYSICAL core count."""
     env = os.environ.get("OMP_NUM_THREADS")
-    return int(env) if env else (os.cpu_count() or 1)
+    if env:
+        return int(env)
+    try:
+        import psutil
+        n = psutil.cpu_count(logical=False)
+        if n:
+            return int(n)
+    except Exception:
+        pass
+    return os.cpu_count() or 1
 
 
 def time_oracle(config, steps, warmup):
@@ -126,6 +144,7 @@ def time_oracle(config, steps, warmup):
     ov, text = ORACLE_SAMPLE[config]
     p = make_problem(config, **ov)
     oracle.build()
+    os.environ.setdefault("OMP_NUM_THREADS", str(_cores()))      # read by the OpenMP runtime when the library first runs
     for _ in range(warmup):
         oracle.run_problem(p)
     t0 = time.perf_counter()
@@ -168,18 +187,26 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     ov = {}
-    if args.positions and args.config == "config4":
+    if args.positions and len(args.config) > 0 and args.config in ("config4", "paper_coarse", "paper_fine"):
         ov["n_pos"] = args.positions
+    if args.sn:
+        ov["sn"] = args.sn
+    if args.pl is not None:
+        ov["pl"] = args.pl
+    from paper_1811_12391_b200 import scan
     p = make_problem(args.config, **ov)
-    # weak scaling: every rank runs the whole workload on its own GPU (independent replicas; a single
-    # projection does not shard, and the scan's per-rank position count is kept fixed)
-    mine = list(range(len(p["sources"])))
+    # A single projection does not shard: every rank runs the whole workload on its own GPU (independent replicas,
+    # weak scaling). The axial scan (config4) shards by source position: rank r takes positions r, r + world, ...,
+    # and the partial dose maps are summed with one all-reduce (strong scaling: the total work is fixed).
+    sharded = world > 1 and len(p["sources"]) > 1 and args.scan == "separate"
+    mine = scan.shard_positions(len(p["sources"]), rank, world) if sharded else list(range(len(p["sources"])))
     m = p["mesh"]
     nv = m["nx"] * m["ny"] * m["nz"]
     M = (p["P_L"] + 1) ** 2
     n_ang = len(p["quadrature"]["w"])
     summed = args.scan == "summed" and len(mine) > 1    # the positions form ONE source, one solve
-    updates_per_step = n_updates(p) // (len(mine) if summed else 1)   # this rank; all ranks do the same amount
+    updates_all = n_updates(p) // (len(p["sources"]) if summed else 1)          # the whole problem
+    job_updates = updates_all if sharded else world * updates_all               # what all ranks together process per step
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
         ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"],
@@ -201,10 +228,10 @@ def run_ours(args):
             step_summed()
             ctx.dos_dose(dose, accumulate=False)
             return
-        for n, s in enumerate(mine):
-            ctx.dos_uncollided(p["sources"][s], p["spectrum"])
-            ctx.dos_solve(p["n_iter"])
-            ctx.dos_dose(dose, accumulate=(n > 0))
+        scan.run_scan(ctx, p, mine, dose)
+        if sharded:
+            with torch.cuda.stream(stream):
+                scan.all_reduce_dose(dose)
 
     def step_e2e():
         ctx.dos_set_material_host(mat_host)
@@ -218,9 +245,16 @@ def run_ours(args):
             if n + 1 < len(mine):
                 ctx.dos_dose(dose, accumulate=(n > 0))
         # the last position's dose is added on the device and the sum is copied to the host
-        if len(mine) > 1:
-            ctx.dos_dose(dose, accumulate=True)
-            dose_pinned.copy_(dose.reshape(-1), non_blocking=False)
+        if len(mine) > 1 or sharded:
+            if mine:
+                ctx.dos_dose(dose, accumulate=(len(mine) > 1))
+            else:
+                dose.zero_()
+            with torch.cuda.stream(stream):           # the context's stream, not torch's current one: the copy must
+                if sharded:                           # come after the last dos_dose
+                    scan.all_reduce_dose(dose)
+                dose_pinned.copy_(dose.reshape(-1), non_blocking=True)
+            stream.synchronize()
         else:
             ctx.dos_dose_host(dose_host, accumulate=False)
 
@@ -274,7 +308,7 @@ def run_ours(args):
     # phase split (one extra untimed-for-the-metric step, CUDA events on the same stream)
     pe = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     pe[0].record(stream)
-    ctx.dos_uncollided(p["sources"][mine[0]], p["spectrum"])
+    ctx.dos_uncollided(p["sources"][mine[0] if mine else 0], p["spectrum"])
     pe[1].record(stream)
     ctx.dos_solve(p["n_iter"])
     pe[2].record(stream)
@@ -290,17 +324,18 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = _peaks()
         sweep_ms = prof["sweep_ms"] / max(prof["sweep_launches"], 1)
-        sweep_bytes = (8 * M + 1) * nv                       # read Q[M], write phi[M] (fp32), 1 B material id
+        sweep_bytes = (12 * M + 1) * nv      # compulsory: read Q_fix[M] + phi_old[M], write phi_new[M] (fp32), 1 B material id
         achieved = sweep_bytes / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
         flop = (4 * M + 12) * nv * n_ang
         rt_ms = prof["raytrace_ms"] / max(prof["raytrace_launches"], 1)
         traffic = None
+        sweep_name = "sweep_umma_kernel" if M >= 25 else "sweep_kernel"     # tensor-memory sweep from P4 up, FFMA sweep below
         tpath = os.path.join(ROOT, "profiles", "traffic.csv")     # ncu dram bytes per launch, copied from profiles/*.md
         if os.path.exists(tpath):
             with open(tpath) as f:
                 for row in f.read().splitlines()[1:]:
                     c = row.split(",")
-                    if len(c) >= 3 and c[0] == args.config and c[1] == "sweep_kernel":
+                    if len(c) >= 3 and c[0] == args.config and c[1] == sweep_name:
                         traffic = int(c[2])
         # FP32 pipe peak: SMs x 128 FP32 lanes x 2 flop x SM clock
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -308,24 +343,26 @@ def run_ours(args):
         alu_peak = sms * 128 * 2 * mhz * 1e6 / 1e12
         tflops = flop / (sweep_ms * 1e-3) / 1e12 if sweep_ms > 0 else 0.0
         line = {
-            "metric": METRIC, "value": world * updates_per_step * args.steps / (total_ms * 1e-3), "unit": UNIT,
+            "metric": METRIC, "value": job_updates * args.steps / (total_ms * 1e-3), "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOADS[args.config] + (" -- summed-source mode: the positions form ONE source, one solve"
                                                              if summed else ""), "positions_per_rank": len(mine),
-                       "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "parallelism": ("source positions sharded over ranks, one all-reduce of the dose map" if sharded else
+                                       "replicas only") if world > 1 else "1 gpu",
                        "l2": "flushed between timed steps (256 MiB fill)", "arithmetic": "fp32 sweep/sources/dose, fp64 ray trace"},
             "dose_map_ms": total_ms / args.steps, "phases_ms": phases, "wall_s_timed_region": wall,
-            "e2e": {"value": world * updates_per_step * args.steps / e2e_total, "unit": UNIT,
+            "e2e": {"value": job_updates * args.steps / e2e_total, "unit": UNIT,
                     "ms_per_step": e2e_total / args.steps * 1e3, "h2d_bytes_per_step": int(nv), "d2h_bytes_per_step": int(4 * nv)},
             "gpu_launches": int(prof["kernel_launches"]),
             "clocks": clocks,
-            "roofline": {"kernel": "sweep_kernel", "bound": "alu", "achieved": tflops, "peak": alu_peak, "unit": "TFLOP/s",
-                         "frac": tflops / alu_peak, "traffic": traffic,
-                         "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 flop x {mhz:.0f} MHz (DESIGN.md section 7)",
-                         "algorithmic_flop_per_launch": flop,
-                         "hbm": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                                 "peak_source": peak_src, "algorithmic_bytes_per_launch": sweep_bytes},
+            "roofline": {"kernel": sweep_name, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": sweep_bytes,
+                         "measured_dram_frac": (traffic / (sweep_ms * 1e-3) / 1e9 / peak) if (traffic and sweep_ms > 0) else None,
+                         "alu": {"achieved": tflops, "peak": alu_peak, "unit": "TFLOP/s", "frac": tflops / alu_peak,
+                                 "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 flop x {mhz:.0f} MHz (DESIGN.md section 7)",
+                                 "algorithmic_flop_per_launch": flop},
                          "launch_ms": sweep_ms,
                          "launches": int(prof["sweep_launches"]), "share_of_step": prof["sweep_ms"] / total_ms if total_ms else None,
                          "updates_per_s_in_kernel": nv * n_ang / (sweep_ms * 1e-3) if sweep_ms > 0 else 0.0},
@@ -350,8 +387,11 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="config2", choices=sorted(WORKLOADS))
-    ap.add_argument("--positions", type=int, default=0, help="config4 only: source positions per step (default 36)")
+    ap.add_argument("--config", default="config5", choices=sorted(WORKLOADS),
+                    help="default: config5, the largest single-GPU workload (BASELINE.json's metric is not quoted on a config)")
+    ap.add_argument("--positions", type=int, default=0, help="config4 / paper_*: source positions per step (default 36 / 16)")
+    ap.add_argument("--sn", type=int, default=0, help="quadrature order override (paper_*: S2..S8)")
+    ap.add_argument("--pl", type=int, default=None, help="scattering order override (paper_*: P0..P1)")
     ap.add_argument("--scan", default="separate", choices=["separate", "summed"],
                     help="config4: one solve per source position with doses summed (default, BASELINE.json), or all "
                          "positions as ONE source and one solve (the paper's CT-scan mode, PAPER.md:69-71)")
@@ -361,6 +401,15 @@ def main():
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # launched without torchrun: spawn the N ranks ourselves, one process per GPU, and relay rank 0's JSON line
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     else:
         run_ours(args)
 

@@ -143,6 +143,19 @@ dos_status dos_uncollided_total(dos_ctx *ctx, float *d_phi_u_out);
  * readings R3, R11, R12), vacuum boundaries, fp32. No convergence test (reading R5). */
 dos_status dos_solve(dos_ctx *ctx, int32_t n_iter);
 
+/* The same with a stopping rule the paper does not state: in each group the source iteration stops
+ * after the first sweep with max_c |phi00^(it) - phi00^(it-1)| <= tol * max_c |phi00^(it)|, or after max_iter sweeps.
+ * h_iters (host [G], may be NULL) receives the sweeps done per group. Synchronises the stream once per sweep (one
+ * 8-byte read-back), so this entry point is NOT enqueue-only. */
+dos_status dos_solve_tol(dos_ctx *ctx, float tol, int32_t max_iter, int32_t *h_iters);
+
+/* Boundary condition of the following solves. reflective_faces: bit 0 the two x faces, bit 1 y, bit 2 z; 0 (default) =
+ * vacuum on all faces. A reflective face returns, in each sweep, the outflow of the mirror-image ordinate
+ * of the PREVIOUS sweep of the same group (lagged; zero in a group's first sweep), which converges to the specular
+ * condition; it is what the infinite-medium check of north_star (phi = Q / (sigma_t - sigma_s0)) needs on the GPU.
+ * Served by the tensor-memory sweep only: DOS_ERR_UNSUPPORTED for a quadrature it has no shape for. */
+dos_status dos_set_boundary(dos_ctx *ctx, int32_t reflective_faces);
+
 /* Scalar fluence per group: collided phi_c^g = phi^g[00] and/or total phi_u^g + phi_c^g.
  * Either pointer may be NULL. device [G][nz][ny][nx] fp32. */
 dos_status dos_fluence(dos_ctx *ctx, float *d_phi_collided, float *d_phi_total);

@@ -16,7 +16,7 @@
 
 struct Layout {
     size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, items_u, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
-        bm2d, bd2m, signs, errflag, um, phi_u_sum, total;
+        bm2d, bd2m, signs, errflag, bx, by, bz, phi00_old, conv, um, phi_u_sum, total;
 };
 
 struct dos_ctx {
@@ -40,6 +40,7 @@ struct dos_ctx {
     dos_source src;
     bool have_dose_acc;
     bool mat_checked;            // the current material grid has been through validate_material_kernel
+    int refl;                    // reflective faces: bit 0 x, 1 y, 2 z (dos_set_boundary); 0 = vacuum
     bool profile, prof_open;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop); kind in ev_kind
     std::vector<int> ev_kind;     // 0 sweep, 1 ray trace
@@ -131,6 +132,13 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.bd2m = take(sizeof(float) * (size_t)2 * NMP * A8);
     l.signs = take(sizeof(unsigned) * (size_t)8 * MP);
     l.errflag = take(sizeof(int) * 4);
+    // reflective boundaries (tensor-memory sweep): two halves (previous / current sweep) of the boundary outflow
+    l.bx = take(sizeof(float) * (size_t)2 * 8 * per * m->nz * m->ny);
+    l.by = take(sizeof(float) * (size_t)2 * 8 * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK);
+    l.bz = take(sizeof(float) * (size_t)2 * 8 * ntj * (m->nx + DOS_FACE_PAD) * per * DOS_TJ);
+    // tolerance-stopped solve: scalar fluence of the previous iterate, two reduction words
+    l.phi00_old = take(sizeof(float) * nv);
+    l.conv = take(sizeof(int) * 4);
     // summed-source mode (dos_uncollided_sum): uncollided moments of all positions and their scalar sum
     l.um = summed ? take(sizeof(float) * G * nv * MP) : 0;
     l.phi_u_sum = summed ? take(sizeof(float) * G * nv) : 0;
@@ -164,7 +172,7 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
 static cudaError_t configure_sweep(dos_ctx *c)
 {
     const bool ffma_ok = dos_sweep_ffma_angles_per_warp(c->per_oct, c->L, 0) != 0;
-    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok && c->MP >= 28) || !ffma_ok;
+    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok && c->MP >= 28) || !ffma_ok || c->refl != 0;
     if (want_umma) {
         if (!c->umma_ok) return cudaErrorInvalidValue;
         int grid = 0;
@@ -264,6 +272,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->umma = false;
     c->grid = c->grid_u = 0;
     c->mat_checked = false;
+    c->refl = 0;
     c->nv = (size_t)mesh->nx * mesh->ny * mesh->nz;
     c->stream = (cudaStream_t)cuda_stream;
     c->d_mat = d_material_ids;
@@ -525,11 +534,14 @@ extern "C" dos_status dos_uncollided_total(dos_ctx *c, float *d_phi_u_out)
     return DOS_OK;
 }
 
-extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
+// n_iter sweeps in every group (tol < 0), or per group until max|phi00 - phi00_old| <= tol max|phi00| with at most
+// n_iter sweeps (tol >= 0; one 8-byte device-to-host read per sweep); h_iters (may be null) [G] receives the counts.
+static dos_status solve_impl(dos_ctx *c, int32_t n_iter, float tol, int32_t *h_iters)
 {
     if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
     if (c->state < 1) return fail(c, DOS_ERR_STATE, "dos_solve before dos_uncollided");
     if (n_iter < 1) return fail(c, DOS_ERR_INVALID_ARG, "n_iter must be >= 1");
+    if (c->refl && !c->umma) return fail(c, DOS_ERR_UNSUPPORTED, "reflective boundaries need the tensor-memory sweep");
     const size_t nvm = c->nv * c->MP;
     float *phi_u = (float *)(c->ws + c->lay.phi_u), *phi_all = (float *)(c->ws + c->lay.phi_all);
     float *qfix = (float *)(c->ws + c->lay.qfix), *q = (float *)(c->ws + c->lay.q);
@@ -554,6 +566,14 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
     u.signs = (const unsigned *)(c->ws + c->lay.signs);
     u.fy = a.fy; u.fz = a.fz; u.done = done; u.queue = queue; u.abort_flag = a.abort_flag;
     const int n_flags = c->umma ? c->n_items_u : c->n_items * c->asplit;
+    // reflective boundaries: halves of the boundary-outflow buffers alternate between "previous sweep" and "this sweep"
+    const size_t bxh = (size_t)8 * c->per_oct * c->mesh.nz * c->mesh.ny, byh = (size_t)8 * c->ntk * (c->mesh.nx + DOS_FACE_PAD) * c->per_oct * DOS_TK,
+                 bzh = (size_t)8 * c->ntj * (c->mesh.nx + DOS_FACE_PAD) * c->per_oct * DOS_TJ;
+    float *bx = (float *)(c->ws + c->lay.bx), *by = (float *)(c->ws + c->lay.by), *bz = (float *)(c->ws + c->lay.bz);
+    float *phi00_old = tol >= 0.f ? (float *)(c->ws + c->lay.phi00_old) : nullptr;
+    int *conv = (int *)(c->ws + c->lay.conv);
+    u.refl = c->refl;
+    int sweep_no = 0;
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
         CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
@@ -562,17 +582,63 @@ extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter)
         c->launches += 1;
         a.phi = u.phi = phi;
         a.sig_t = u.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
-        for (int it = 0; it < n_iter; ++it) {
+        if (c->refl) {
+            // every group starts from zero boundary inflow (the lagged reflective condition of the first sweep)
+            CUDA_TRY(c, cudaMemsetAsync(bx, 0, sizeof(float) * 2 * bxh, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(by, 0, sizeof(float) * 2 * byh, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(bz, 0, sizeof(float) * 2 * bzh, c->stream));
+        }
+        int it = 0;
+        for (; it < n_iter; ++it) {
             CUDA_TRY(c, dos_launch_source_update(c->nv, c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, sig_s, qfix, phi, q, it == 0,
-                                                 done, n_flags, queue, c->stream));
+                                                 done, n_flags, queue, phi00_old, c->stream));
+            const int cur = sweep_no & 1, prv = cur ^ 1;
+            u.bx_in = bx + prv * bxh; u.bx_out = bx + cur * bxh;
+            u.by_in = by + prv * byh; u.by_out = by + cur * byh;
+            u.bz_in = bz + prv * bzh; u.bz_out = bz + cur * bzh;
+            ++sweep_no;
             prof_begin(c, 0);
             if (c->umma) CUDA_TRY(c, dos_launch_sweep_umma(u, c->L, c->grid_u, c->stream));
             else CUDA_TRY(c, dos_launch_sweep_ffma(a, c->L, c->ag, c->grid, c->two_per_sm, c->stream));
             prof_end(c);
             c->launches += 2;
+            if (tol >= 0.f) {
+                int h[2] = {0, 0};
+                CUDA_TRY(c, dos_launch_conv(c->nv, c->MP, phi, phi00_old, conv, c->stream));
+                CUDA_TRY(c, cudaMemcpyAsync(h, conv, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+                CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+                c->launches += 1;
+                float d, m;
+                std::memcpy(&d, &h[0], 4); std::memcpy(&m, &h[1], 4);
+                if (d <= tol * m) { ++it; break; }
+            }
         }
+        if (h_iters) h_iters[g] = it;
     }
     c->state = 2;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_solve(dos_ctx *c, int32_t n_iter) { return solve_impl(c, n_iter, -1.f, nullptr); }
+
+extern "C" dos_status dos_solve_tol(dos_ctx *c, float tol, int32_t max_iter, int32_t *h_iters)
+{
+    if (!(tol >= 0.f)) return fail(c, DOS_ERR_INVALID_ARG, "tol must be >= 0");
+    return solve_impl(c, max_iter, tol, h_iters);
+}
+
+extern "C" dos_status dos_set_boundary(dos_ctx *c, int32_t reflective_faces)
+{
+    if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
+    if (reflective_faces < 0 || reflective_faces > 7) return fail(c, DOS_ERR_INVALID_ARG, "reflective_faces is a 3-bit mask (x, y, z)");
+    if (reflective_faces && !c->umma_ok) return fail(c, DOS_ERR_UNSUPPORTED, "reflective boundaries need the tensor-memory sweep, which has no shape for this quadrature");
+    const int old = c->refl;
+    c->refl = reflective_faces;
+    if (configure_sweep(c) != cudaSuccess) {
+        c->refl = old;
+        configure_sweep(c);
+        return fail(c, DOS_ERR_UNSUPPORTED, "reflective boundaries: no admissible sweep");
+    }
     return DOS_OK;
 }
 

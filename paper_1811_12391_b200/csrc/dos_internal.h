@@ -82,6 +82,15 @@ struct SweepUArgs {
     int *done;               // [2 * ntj * ntk (by quad, tile)] steps finished and published
     int *queue;              // work-queue head
     int *abort_flag;
+    // reflective boundaries (lagged: the inflow of an ordinate is the outflow of its mirror image in the
+    // previous sweep). refl bit 0 / 1 / 2: x / y / z faces. The boundary fluxes of sweep s live in half (s & 1):
+    const float *bx_in;      // [8][A][nz][ny]   x-boundary outflow of the previous sweep (octant, angle, k, j: global indices)
+    float *bx_out;           //                  ... of this sweep
+    const float *by_in;      // [8][ntk][nx + PAD][A][TK]  y-boundary outflow of the previous sweep, tile-face layout (by diagonal)
+    float *by_out;
+    const float *bz_in;      // [8][ntj][nx + PAD][A][TJ]
+    float *bz_out;
+    int refl;
 };
 int dos_sweep_umma_supported(int per_oct, int L);
 cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int *grid_out);

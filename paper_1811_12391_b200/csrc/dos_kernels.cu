@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(256) source_update_kernel(size_t nv, int MV, i
                                                             int n_mat, int G, int n_leg, int g, const float *__restrict__ sig_s,
                                                             const float4 *__restrict__ qfix, float4 *__restrict__ phi,
                                                             float4 *__restrict__ q, int first, int *done, int n_flags,
-                                                            int *queue)
+                                                            int *queue, float *__restrict__ phi00_old)
 {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t < (size_t)n_flags) done[t] = 0;
@@ -230,6 +230,7 @@ __global__ void __launch_bounds__(256) source_update_kernel(size_t nv, int MV, i
     const size_t cell = t / MV;
     const int v = (int)(t - cell * MV);
     float4 out = qfix[t];
+    if (phi00_old && v == 0) phi00_old[cell] = first ? 0.f : phi[t].x;      // scalar fluence of the previous iterate (dos_solve_tol)
     if (!first) {
         const float *ss = sig_s + (size_t)min((int)mat[cell], n_mat - 1) * (n_leg + 1) * G * G + (size_t)g * G + g;   // + l*G*G
         const float4 p = phi[t];
@@ -295,14 +296,46 @@ cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const 
 
 cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int n_mat, int G, int n_leg, int L, int g, const float *sig_s,
                                      const float *qfix, float *phi, float *q, int first, int *done, int n_flags,
-                                     int *queue, cudaStream_t st)
+                                     int *queue, float *phi00_old, cudaStream_t st)
 {
     const int M = (L + 1) * (L + 1), MV = dos_mpad(L) / 4;
     size_t n = nv * MV;
     if ((size_t)n_flags > n) n = (size_t)n_flags;
     const unsigned grid = (unsigned)((n + 255) / 256);
     source_update_kernel<<<grid, 256, 0, st>>>(nv, MV, M, mat, n_mat, G, n_leg, g, sig_s, (const float4 *)qfix, (float4 *)phi,
-                                               (float4 *)q, first, done, n_flags, queue);
+                                               (float4 *)q, first, done, n_flags, queue, phi00_old);
+    return cudaGetLastError();
+}
+
+// Stopping measure of dos_solve_tol: out[0] = max_c |phi00_new - phi00_old|, out[1] = max_c |phi00_new| (as the bit
+// patterns of non-negative floats, which order like integers; out must be zeroed before the launch).
+namespace {
+__global__ void __launch_bounds__(256) conv_kernel(size_t nv, int MP, const float *__restrict__ phi, const float *__restrict__ phi00_old, int *out)
+{
+    float d = 0.f, a = 0.f;
+    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < nv; c += (size_t)gridDim.x * blockDim.x) {
+        const float v = phi[c * MP];
+        d = fmaxf(d, fabsf(v - phi00_old[c]));
+        a = fmaxf(a, fabsf(v));
+    }
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        d = fmaxf(d, __shfl_xor_sync(0xffffffffu, d, s));
+        a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, s));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(out, __float_as_int(d));
+        atomicMax(out + 1, __float_as_int(a));
+    }
+}
+}  // namespace
+
+cudaError_t dos_launch_conv(size_t nv, int MP, const float *phi, const float *phi00_old, int *out2, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(out2, 0, 2 * sizeof(int), st);
+    if (e != cudaSuccess) return e;
+    const unsigned grid = (unsigned)((nv + 255) / 256 < 1184 ? (nv + 255) / 256 : 1184);
+    conv_kernel<<<grid, 256, 0, st>>>(nv, MP, phi, phi00_old, out2);
     return cudaGetLastError();
 }
 

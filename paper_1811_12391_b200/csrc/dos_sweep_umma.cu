@@ -244,7 +244,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
         const int packed = p.items[item];
         quad = packed & 7; tj = (packed >> 3) & 0x3FFF; tk = packed >> 17;
         fid = (quad * p.ntk + tk) * p.ntj + tj;      // hand-off flag of this (quad, tile)
-        has_y = tj > 0; has_z = tk > 0;
+        has_y = tj > 0 || (p.refl & 2); has_z = tk > 0 || (p.refl & 4);      // there is y / z inflow to stage (else vacuum)
 #if DOS_UMMA_TRACE
         trace_on = item == 601;
 #endif
@@ -254,10 +254,11 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
     if (is_service) {
         while (next_item()) {
             // ------- service warp: publishes this item's progress, follows the two upwind items' progress -------
-            const int *up_y = p.done + (has_y ? fid - 1 : fid), *up_z = p.done + (has_z ? fid - p.ntj : fid);
+            const bool up_tile_y = tj > 0, up_tile_z = tk > 0;       // boundary inflow (reflective) needs no hand-off
+            const int *up_y = p.done + (up_tile_y ? fid - 1 : fid), *up_z = p.done + (up_tile_z ? fid - p.ntj : fid);
             int *my_flag = p.done + fid;
-            int avail_y = has_y ? 0 : BIG, avail_z = has_z ? 0 : BIG;
-            if (lane == 0) s_allowed = (has_y || has_z) ? -1 : BIG;
+            int avail_y = up_tile_y ? 0 : BIG, avail_z = up_tile_z ? 0 : BIG;
+            if (lane == 0) s_allowed = (up_tile_y || up_tile_z) ? -1 : BIG;
             __syncthreads();                          // S2
             int published = 0, spins = 0;
             for (;;) {
@@ -300,9 +301,13 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             __syncthreads();                          // S2: s_allowed in place
             if (has_y || has_z) {
                 const int qq = lane & 3, which = lane >> 2;       // lanes 0..7: (octant, y / z)
-                const int oid = ((quad * 4 + qq) * p.ntk + tk) * p.ntj + tj;
+                const int oo = quad * 4 + qq;
+                const int oid = (oo * p.ntk + tk) * p.ntj + tj;
                 const bool mine = lane < 8 && (which == 0 ? has_y : has_z);
-                const float *src = which == 0 ? p.fy + (size_t)(oid - 1) * fstride_y : p.fz + (size_t)(oid - p.ntj) * fstride_z;
+                // upwind tile's face buffer -- or, on a reflective mesh boundary, what the mirror octant's last tile
+                // wrote there in the previous sweep (same layout: the boundary is a virtual upwind tile)
+                const float *src = which == 0 ? (tj > 0 ? p.fy + (size_t)(oid - 1) * fstride_y : p.by_in + (size_t)((oo ^ 2) * p.ntk + tk) * fstride_y)
+                                              : (tk > 0 ? p.fz + (size_t)(oid - p.ntj) * fstride_z : p.bz_in + (size_t)((oo ^ 4) * p.ntj + tj) * fstride_z);
                 const int blk = which == 0 ? A * DOS_TK : A * DOS_TJ;                  // floats per step
                 float *dst0 = which == 0 ? s_finy + qq * blk : s_finz + qq * blk;
                 const unsigned bytes_all = (unsigned)((has_y ? 4 * A * DOS_TK : 0) + (has_z ? 4 * A * DOS_TJ : 0)) * 4u;
@@ -409,11 +414,17 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             const int grp = warp >> 2, a0 = grp * AG;
             const int jj = lane & (DOS_TJ - 1), kk = lane / DOS_TJ;
             const bool in_y = jj == 0, in_z = kk == 0;
-            const bool store_y = g.valid && jj == DOS_TJ - 1 && tj < p.ntj - 1;
-            const bool store_z = g.valid && kk == DOS_TK - 1 && tk < p.ntk - 1;
+            // the tile's last j / k lanes hand their outflow to the downwind tile; on the mesh's last tile row (ragged:
+            // lane (ny - 1) % 8 / (nz - 1) % 4) to the reflective boundary buffer, or nowhere (vacuum)
+            const bool last_tj = tj == p.ntj - 1, last_tk = tk == p.ntk - 1;
+            const int jst = last_tj ? (p.ny - 1) % DOS_TJ : DOS_TJ - 1, kst = last_tk ? (p.nz - 1) % DOS_TK : DOS_TK - 1;
+            const bool store_y = g.valid && jj == jst && (!last_tj || (p.refl & 2));
+            const bool store_z = g.valid && kk == kst && (!last_tk || (p.refl & 4));
             const int oid = (o * p.ntk + tk) * p.ntj + tj;
-            float *fy_st = p.fy + (size_t)oid * fstride_y + kk + ((long long)(1 - DOS_TJ) * A + a0) * DOS_TK;
-            float *fz_st = p.fz + (size_t)oid * fstride_z + jj + ((long long)(1 - DOS_TK) * A + a0) * DOS_TJ;
+            float *fy_st = (last_tj ? p.by_out + (size_t)(o * p.ntk + tk) * fstride_y : p.fy + (size_t)oid * fstride_y) + kk +
+                           ((long long)(-jst) * A + a0) * DOS_TK;
+            float *fz_st = (last_tk ? p.bz_out + (size_t)(o * p.ntj + tj) * fstride_z : p.fz + (size_t)oid * fstride_z) + jj +
+                           ((long long)(-kst) * A + a0) * DOS_TJ;
             const int fy_inc = A * DOS_TK, fz_inc = A * DOS_TJ;
             const float *finy = s_finy + (q * A + a0) * DOS_TK + kk, *finz = s_finz + (q * A + a0) * DOS_TJ + jj;
             const uint8_t *mat_p = p.mat + g.cbase;
@@ -476,9 +487,19 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 if (lane == 0) mbar_arrive(&phi_empty[gsx % DPS]);
             };
 
+            // x faces: the column's inflow is vacuum or the mirror octant's outflow of the previous sweep
+            // (reflective); px starts as that inflow and is only touched while the lane is active
+            const int jp_ = tj * DOS_TJ + jj, kp_ = tk * DOS_TK + kk;
+            const int jg = (o & 2) ? p.ny - 1 - jp_ : jp_, kg = (o & 4) ? p.nz - 1 - kp_ : kp_;
+            const size_t bxi = g.valid ? (size_t)kg * p.ny + jg : 0, bxs = (size_t)p.nz * p.ny;
+            const bool refl_x = (p.refl & 1) && g.valid;
+            const int t_last = g.valid ? t_lo + nx - 1 : -1;
             float px[AG], oy[AG], oz[AG];
 #pragma unroll
-            for (int r = 0; r < AG; ++r) px[r] = oy[r] = oz[r] = 0.f;
+            for (int r = 0; r < AG; ++r) {
+                px[r] = refl_x ? __ldcg(p.bx_in + ((size_t)(o ^ 1) * A + a0 + r) * bxs + bxi) : 0.f;
+                oy[r] = oz[r] = 0.f;
+            }
             auto mat_of = [&](int s) -> int { return ((unsigned)(s - t_lo) < (unsigned)nx) ? min((int)__ldg(mat_p + (long long)istep * s), p.n_mat - 1) : 0; };
             int m_cur = mat_of(0), m_nxt = mat_of(1);
             for (int s = 0; s < LA && s < T; ++s) stage(s);
@@ -502,7 +523,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 const int fslot = (int)(fs % RFU) * 4 * A;
                 const float *rden = s_rden + m0 * A + a0;
                 const float sig0 = s_sig[m0];
-                const bool first_x = t == t_lo;
+                const bool last_x = refl_x && t == t_last;
                 const unsigned tq = tm_dq + lane_base + (gs % DQS) * NAP + a0;            // D_q columns of this warp's angles
                 const unsigned tp = tm_psi + lane_base + (gs % PSL) * 2 * A8 + a0;        // psi operand columns (hi; lo at + A8)
                 // The AG angles go in chunks of CH. Inside a chunk everything is straight-line code (selects, no branches),
@@ -528,7 +549,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                         if (in_y) yin = has_y ? finy[fslot * DOS_TK + r * DOS_TK] : 0.f;        // tile inflow or vacuum
                         if (in_z) zin = has_z ? finz[fslot * DOS_TJ + r * DOS_TJ] : 0.f;
                         const float4 cc = cdd4[r];
-                        ix[e] = first_x ? 0.f : px[r];
+                        ix[e] = px[r];
                         yi[e] = yin; zi[e] = zin;
                         const float num = fmaf(cc.x, ix[e], fmaf(cc.y, yin, fmaf(cc.z, zin, qd[e])));
                         const float c = (DOS_UMMA_ABL & 8) ? 0.f : num * rden[r];
@@ -561,6 +582,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                             px[r] = ox[e]; oy[r] = oyr[e]; oz[r] = ozr[e];
                             if (store_y) __stcg(fy_st + r * DOS_TK, oyr[e]);
                             if (store_z) __stcg(fz_st + r * DOS_TJ, ozr[e]);
+                            if (last_x) __stcg(p.bx_out + ((size_t)o * A + a0 + r) * bxs + bxi, ox[e]);
                         }
                         tf32_split(act ? pc[e] : 0.f, hi[e], lo[e]);
                     }

@@ -21,7 +21,7 @@ STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_
           -5: "DOS_ERR_CUDA", -6: "DOS_ERR_UNSUPPORTED"}
 
 EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_sum",
-           "dos_uncollided_total", "dos_solve", "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option",
+           "dos_uncollided_total", "dos_solve", "dos_solve_tol", "dos_set_boundary", "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option",
            "dos_profile", "dos_profile_reset", "dos_destroy", "dos_last_error"]
 
 
@@ -63,6 +63,10 @@ _lib.dos_uncollided_sum.restype = C.c_int
 _lib.dos_uncollided_sum.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
 _lib.dos_solve.restype = C.c_int
 _lib.dos_solve.argtypes = [C.c_void_p, C.c_int32]
+_lib.dos_solve_tol.restype = C.c_int
+_lib.dos_solve_tol.argtypes = [C.c_void_p, C.c_float, C.c_int32, C.c_void_p]
+_lib.dos_set_boundary.restype = C.c_int
+_lib.dos_set_boundary.argtypes = [C.c_void_p, C.c_int32]
 _lib.dos_fluence.restype = C.c_int
 _lib.dos_fluence.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.dos_dose.restype = C.c_int
@@ -198,6 +202,15 @@ class Context:
 
     def dos_solve(self, n_iter):
         self._check(_lib.dos_solve(self.handle, int(n_iter)))
+
+    def dos_solve_tol(self, tol, max_iter):
+        """Returns the sweeps done per group (numpy int32 [G])."""
+        iters = np.zeros(self.G, dtype=np.int32)
+        self._check(_lib.dos_solve_tol(self.handle, float(tol), int(max_iter), iters.ctypes.data))
+        return iters
+
+    def dos_set_boundary(self, reflective_faces):
+        self._check(_lib.dos_set_boundary(self.handle, int(reflective_faces)))
 
     def dos_fluence(self, phi_collided=None, phi_total=None):
         self._check(_lib.dos_fluence(self.handle, phi_collided.data_ptr() if phi_collided is not None else None,

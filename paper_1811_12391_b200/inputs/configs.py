@@ -1,4 +1,5 @@
-"""The five BASELINE.json workloads as seeded synthetic problems (SURVEY.md 8(d) recipe).
+"""The five BASELINE.json workloads, and the paper-shaped workload of SURVEY.md 8(f) N4, as seeded synthetic problems
+(SURVEY.md 8(d) recipe).
 
 `make_problem(name)` returns a plain dict of numpy arrays / scalars; the same dict feeds the oracle
 (tests, bench cpu_baseline) and the CUDA library. No transport arithmetic lives here.
@@ -17,12 +18,21 @@ def _source(pos, axis, up, tan_half_fan, tan_half_cone, isotropic):
             "tan_half_cone": float(tan_half_cone), "isotropic": int(isotropic)}
 
 
-def scan_source(theta: float, radius: float = 54.0):
-    """Cone-beam source on a circle of `radius` cm in the z = 0 plane, axis pointing at the origin,
-    4 cm axial collimation at the isocentre (tan_half_cone = 2/54), 21 degree half fan."""
+def scan_source(theta: float, radius: float = 54.0, tan_half_fan=None, tan_half_cone=None):
+    """Cone-beam source on a circle of `radius` cm in the z = 0 plane, axis pointing at the origin; by default
+    4 cm axial collimation at the isocentre (tan_half_cone = 2/54) and a 21 degree half fan."""
     c, s = math.cos(theta), math.sin(theta)
     return _source((radius * c, radius * s, 0.0), (-c, -s, 0.0), (0.0, 0.0, 1.0),
-                   math.tan(math.radians(21.0)), 2.0 / 54.0, 0)
+                   math.tan(math.radians(21.0)) if tan_half_fan is None else tan_half_fan,
+                   2.0 / 54.0 if tan_half_cone is None else tan_half_cone, 0)
+
+
+# SURVEY.md 8(f) N4: the SHAPE of the paper's own workload (PAPER.md:75-81; BASELINE.md "What the paper reports"):
+# 7 energy groups with edges 100/75/70/60/45/30/20/10 keV, a 100 kVp spectrum, a 35 cm water cylinder in a
+# 50 x 50 x 12.5 cm box on a 64x64x16 ("coarse", 7.81 mm) or 256x256x64 ("fine", 1.95 mm) mesh, S2-S8 x P0-P1
+# (default S6/P0, the setting of the paper's CT-scan runs and of its Table 6), 16 source positions, 30 degree cone.
+# The cross sections, spectrum and phantom are the synthetic stand-ins of this package, not the paper's data.
+PAPER_EDGES = (100.0, 75.0, 70.0, 60.0, 45.0, 30.0, 20.0, 10.0)
 
 
 _SPECS = {
@@ -32,6 +42,8 @@ _SPECS = {
     "config3": (128, 128, 64, 0.3, 19, 16, 5, 20, "cylinder", 1),
     "config4": (256, 256, 64, 0.15, 19, 8, 3, 15, "abdomen", 36),
     "config5": (256, 256, 256, 0.14, 19, 16, 5, 20, "abdomen", 1),
+    "paper_coarse": (64, 64, 16, 50.0 / 64, 7, 6, 0, 20, "paper_cylinder", 16),
+    "paper_fine": (256, 256, 64, 50.0 / 256, 7, 6, 0, 20, "paper_cylinder", 16),
 }
 
 
@@ -62,6 +74,15 @@ def make_problem(name: str, **override):
         table = xs.make_xs(mats, n_group, 120.0, 10.0, pl)
         spectrum = xs.kramers_spectrum(n_group, 120.0, 10.0, seed=1)
         sources = [scan_source(0.5 * math.pi)]                    # (0, 54, 0), axis (0, -1, 0)
+    elif kind == "paper_cylinder":
+        if n_group != 7:
+            raise ValueError("the paper-shaped workload has the paper's 7 groups")
+        mats = ["air", "water"]
+        mat = phantoms.cylinder(nx, ny, nz, vox, vox, vox, radius=17.5)
+        table = xs.make_xs(mats, 7, 100.0, 10.0, pl, edges=PAPER_EDGES)
+        spectrum = xs.kramers_spectrum(7, 100.0, 10.0, kvp=100.0, seed=1, edges=PAPER_EDGES)
+        t15 = math.tan(math.radians(15.0))                       # "30 degree cone": 15 degree half angles both ways
+        sources = [scan_source(2.0 * math.pi * q / n_pos, tan_half_fan=t15, tan_half_cone=t15) for q in range(n_pos)]
     else:
         mats = phantoms.ABDOMEN_MATERIALS
         mat = phantoms.abdomen(nx, ny, nz, seed=3)

@@ -55,16 +55,18 @@ def _legendre_table(n_leg: int, x: np.ndarray) -> np.ndarray:
 
 
 def make_xs(material_names, n_group: int, e_hi: float, e_lo: float, n_leg: int,
-            n_e_nodes: int = 16, n_mu_nodes: int = 128):
+            n_e_nodes: int = 16, n_mu_nodes: int = 128, edges=None):
     """Multigroup table for the listed materials.
 
     Returns dict with float32 arrays
       sigma_t [n_mat][G]                 1/cm
       sigma_s [n_mat][n_leg+1][G][G]     [from][to], zero for to < from (downscatter only; eq. 2)
       kerma   [n_mat][G]                 keV cm^2 / g  (collision kerma per unit fluence), air row = 0
-    and 'edges' (float64, descending).
+    and 'edges' (float64, descending). `edges` (G+1 descending values, keV) replaces the uniform-width structure,
+    e.g. the paper's 7 groups 100/75/70/60/45/30/20/10 keV.
     """
-    edges = group_edges(n_group, e_hi, e_lo)
+    edges = group_edges(n_group, e_hi, e_lo) if edges is None else np.asarray(edges, dtype=np.float64)
+    assert edges.shape == (n_group + 1,) and np.all(np.diff(edges) < 0)
     xe, we = np.polynomial.legendre.leggauss(n_e_nodes)
     xm, wm = np.polynomial.legendre.leggauss(n_mu_nodes)
     pl = _legendre_table(n_leg, xm)                           # [l][mu-node]
@@ -103,9 +105,9 @@ def uniform_spectrum(n_group: int) -> np.ndarray:
 
 
 def kramers_spectrum(n_group: int, e_hi: float, e_lo: float, kvp: float = 120.0, al_cm: float = 0.2,
-                     seed: int = 1, n_e_nodes: int = 16) -> np.ndarray:
+                     seed: int = 1, n_e_nodes: int = 16, edges=None) -> np.ndarray:
     """Seeded synthetic Kramers spectrum with Al filtration, group-integrated, sum = 1."""
-    edges = group_edges(n_group, e_hi, e_lo)
+    edges = group_edges(n_group, e_hi, e_lo) if edges is None else np.asarray(edges, dtype=np.float64)
     xe, we = np.polynomial.legendre.leggauss(n_e_nodes)
     _, ne23, _ = MATERIALS["aluminium"]
     s = np.zeros(n_group)

@@ -133,3 +133,19 @@ def test_null_context_calls_return_status():
     assert lib.dos_uncollided(None, None, None, None) == -1
     assert lib.dos_check(None) == -1
     lib.dos_destroy(None)                                        # no-op
+
+
+def test_paper_shaped_workload_has_the_papers_shape():
+    """7 groups with edges 100/75/70/60/45/30/20/10 keV, a 50 x 50 x 12.5 cm box on
+    64x64x16 or 256x256x64 voxels, 16 source positions, S6/P0 by default; spectrum normalised per source particle."""
+    import numpy as np
+    from paper_1811_12391_b200.inputs import make_problem
+    p = make_problem("paper_coarse")
+    m = p["mesh"]
+    assert (m["nx"], m["ny"], m["nz"]) == (64, 64, 16) and abs(m["nx"] * m["dx"] - 50.0) < 1e-12 and abs(m["nz"] * m["dz"] - 12.5) < 1e-12
+    assert list(p["edges"]) == [100.0, 75.0, 70.0, 60.0, 45.0, 30.0, 20.0, 10.0] and p["n_group"] == 7
+    assert len(p["sources"]) == 16 and len(p["quadrature"]["w"]) == 48 and p["P_L"] == 0
+    assert abs(float(np.sum(p["spectrum"], dtype=np.float64)) - 1.0) < 1e-6
+    assert p["sigma_s"].shape == (2, 1, 7, 7) and np.all(np.triu(p["sigma_s"][1, 0]) == p["sigma_s"][1, 0])    # downscatter only
+    f = make_problem("paper_fine", n_pos=1)
+    assert (f["mesh"]["nx"], f["mesh"]["nz"]) == (256, 64) and abs(f["mesh"]["dx"] - 50.0 / 256) < 1e-12

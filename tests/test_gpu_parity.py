@@ -212,6 +212,95 @@ def test_config5_full_mesh_properties(dos, orc):
     ctx.close()
 
 
+# ------------------------------------------------- reflective boundaries, stopping rule --
+def test_reflective_boundaries_parity_and_balance(dos, orc):
+    """dos_set_boundary (PAPER.md:41 states vacuum; north_star check 2 needs reflective faces). (a) GPU vs the oracle's
+    lagged reflective option on a ragged multi-tile mesh, S8/P3 and S16/P5, a few iterations: every octant's boundary
+    outflow must reach its mirror octant at the right cell, angle and sweep. (b) With all faces reflective nothing
+    leaks, so at convergence absorption = source, group by group: sum_c (sigma_t - sigma_s0^{g->g}) phi_c^g =
+    sum_c [sum_{g'<=g} sigma_s0^{g'->g} phi_u^{g'} + sum_{g'<g} sigma_s0^{g'->g} phi_c^{g'}] (north_star check 3 on the
+    GPU, homogeneous water so that sigma is one number per group)."""
+    for name, ov in (("config2", dict(nx=21, ny=13, nz=10, voxel=1.6, n_group=3, n_iter=5)),
+                     ("config3", dict(nx=12, ny=17, nz=6, voxel=2.5, n_group=2, n_iter=4))):
+        p = _make(name, **ov)
+        src = p["sources"][0]
+        pu = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+        pc_ref, pabs = orc.solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"], p["n_iter"],
+                                 source_pos=src["pos"], phi_u=pu, reflective=True, want_abs=True)
+        ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+        ctx.dos_set_boundary(7)
+        pc = ctx.new_field()
+        ctx.dos_uncollided(src, p["spectrum"])
+        ctx.dos_solve(p["n_iter"])
+        ctx.dos_fluence(pc, None)
+        ctx.dos_check()
+        assert_fluence_parity(pc.cpu().numpy(), pc_ref[:, 0], f"{name} reflective collided fluence", scale=pabs)
+        # back to vacuum on the same context: the vacuum result of a fresh context
+        ctx.dos_set_boundary(0)
+        ctx.dos_uncollided(src, p["spectrum"])
+        ctx.dos_solve(p["n_iter"])
+        ctx.dos_fluence(pc, None)
+        vac = dos.run_problem(p)["phi_c"]
+        assert np.abs(pc.cpu().numpy() - vac).max() <= 2e-6 * np.abs(vac).max()
+        ctx.close()
+    # (b) balance in a closed water box
+    p = _make("config1", nx=10, ny=9, nz=6, n_iter=150)
+    src = p["sources"][0]
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    ctx.dos_set_boundary(7)
+    pu, pc = ctx.new_field(), ctx.new_field()
+    ctx.dos_uncollided(src, p["spectrum"], pu)
+    ctx.dos_solve(p["n_iter"])
+    ctx.dos_fluence(pc, None)
+    ctx.dos_check()
+    ctx.close()
+    su = pu.double().sum(dim=(1, 2, 3)).cpu().numpy()
+    sc = pc.double().sum(dim=(1, 2, 3)).cpu().numpy()
+    st, s0 = p["sigma_t"][0].astype(float), p["sigma_s"][0, 0].astype(float)       # water; [from][to]
+    for g in range(p["n_group"]):
+        source = sum(s0[gp, g] * su[gp] for gp in range(g + 1)) + sum(s0[gp, g] * sc[gp] for gp in range(g))
+        assert abs((st[g] - s0[g, g]) * sc[g] - source) <= 2e-5 * source, g
+
+
+def test_solve_with_stopping_rule(dos, orc):
+    """dos_solve_tol: per-group iteration counts come back; the oracle run with exactly those counts agrees at the
+    parity tolerances, its own stopping measure at the last sweep is at or below tol (up to fp32 noise) and, one sweep
+    earlier, above it -- both sides take the same decision although one tests in fp32 and the other in fp64."""
+    p = _make("config2", nx=27, ny=19, nz=9, voxel=1.4, n_group=5, n_iter=40)
+    src = p["sources"][0]
+    tol = 2e-3
+    ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+    pc = ctx.new_field()
+    ctx.dos_uncollided(src, p["spectrum"])
+    iters = ctx.dos_solve_tol(tol, p["n_iter"])
+    ctx.dos_fluence(pc, None)
+    ctx.dos_check()
+    ctx.close()
+    assert iters.min() >= 1 and iters.max() < p["n_iter"] and len(set(iters.tolist())) > 1, iters
+    pu = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], src, p["spectrum"])
+    args = (p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"])
+    ref, conv = orc.solve(*args, 1, source_pos=src["pos"], phi_u=pu, n_iter_g=iters, want_conv=True)
+    l2, mx = per_group_errors(pc.cpu().numpy(), ref[:, 0])
+    assert l2 <= 1e-5, l2
+    assert (conv <= tol * 1.01).all(), (conv, iters)
+    # one sweep fewer in a group leaves its measure above tol (the rule stops at the FIRST sweep that meets it)
+    g = int(np.argmax(iters))
+    fewer = iters.copy()
+    fewer[g] -= 1
+    _, conv2 = orc.solve(*args, 1, source_pos=src["pos"], phi_u=pu, n_iter_g=fewer, want_conv=True)
+    assert conv2[g] > tol * 0.99
+
+
+def test_paper_shaped_workload_parity(dos, orc):
+    """the paper's 7-group structure, S6/P0 and S4/P1, 30 degree cone, several positions as ONE source
+    (the paper's CT-scan mode), on a reduced mesh of the 50 x 50 x 12.5 cm box."""
+    for sn, pl in ((6, 0), (4, 1), (8, 1)):
+        p = _make("paper_coarse", nx=26, ny=26, nz=7, voxel=50.0 / 26, n_iter=4, n_pos=4, sn=sn, pl=pl)
+        assert_problem_parity(dos.run_problem_summed(p), orc.run_problem_summed(p), f"paper-shaped S{sn}/P{pl}, 4 positions summed")
+    p = _make("paper_coarse", nx=26, ny=26, nz=7, voxel=50.0 / 26, n_iter=5, n_pos=1)
+    assert_problem_parity(dos.run_problem(p), orc.run_problem(p), "paper-shaped S6/P0 single projection")
+
+
 # ------------------------------------------------------------------------------ method properties --
 def test_uncollided_independent_of_quadrature_and_order(dos):
     """phi_u does not involve S_N or P_L -> bit-identical across them."""
