@@ -84,8 +84,11 @@ typedef struct {
     int32_t isotropic;
 } dos_source;
 
-/* Bytes of device workspace dos_create needs for this problem. n_batch = 1: one source per solve; n_batch > 1:
- * also the buffers of the summed-source mode (dos_uncollided_sum): [G][Nv][MP] + [G][Nv] floats more. */
+/* Bytes of device workspace dos_create needs for this problem. n_batch (1..64) = source positions that can be in flight
+ * at once: dos_uncollided_batch traces up to n_batch positions and dos_solve then sweeps them together (SURVEY.md 8(f)
+ * N2); each position owns its own uncollided fluence, moments of all groups, sweep source and face buffers (a "slot").
+ * n_batch > 1 also adds the buffers of the summed-source mode (dos_uncollided_sum): [G][Nv][MP] + [G][Nv] floats.
+ * dos_create reads the slot count back from the size of the workspace it is given. */
 dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs, const dos_quadrature *quad,
                                int32_t P_L, int32_t n_batch, size_t *bytes_out);
 
@@ -118,6 +121,16 @@ dos_status dos_set_material_host(dos_ctx *ctx, const uint8_t *h_material_ids);
  *   d_phi_u_out     device [G][nz][ny][nx] or NULL: also copy the result there                      */
 dos_status dos_uncollided(dos_ctx *ctx, const dos_source *source, const float *spectrum,
                           float *d_phi_u_out);
+
+/* Position batch (BASELINE.json config 4: an axial scan is a set of independent problems on one mesh):
+ * the uncollided fluence of n_sources positions (host array; 1 <= n_sources <= the n_batch the workspace was sized for),
+ * one slot each. The following dos_solve sweeps all of them in the SAME launches -- the work queue of a sweep holds the
+ * (position, octant, tile) items of every position, so that small meshes fill the SMs and the tile-wavefront tail of one
+ * position overlaps the head of the next; results are those of separate solves, bit for bit up to the order of the
+ * moment reductions. dos_fluence then fills [n_sources][G][nz][ny][nx], dos_dose returns the SUM of the positions' dose
+ * maps (a9). d_phi_u_out: device [n_sources][G][nz][ny][nx] or NULL. */
+dos_status dos_uncollided_batch(dos_ctx *ctx, int32_t n_sources, const dos_source *sources, const float *spectrum,
+                                float *d_phi_u_out);
 
 /* Summed-source mode (the cone beams of a CT scan form ONE source and
  * the S_N equations are solved once). Like dos_uncollided, but the uncollided fluence of this source is ADDED to

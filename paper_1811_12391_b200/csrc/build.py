@@ -12,7 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SOURCES = ["dos_api.cu", "dos_kernels.cu", "dos_sweep_umma.cu", "dos_sweep_ffma.cu"]
 HEADERS = ["dos_internal.h", "dos_kernels.h", "dos_sm100.cuh", os.path.join("..", "..", "include", "dos.h")]
 LIB = os.path.join(HERE, "libdos.so")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++20", "-Xcompiler", "-fPIC"]
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-Xcompiler", "-fPIC"]
+STD = {"dos_sweep_umma.cu": "-std=c++20"}     # templated lambdas; nvcc 12.9 breaks on libstdc++ 13 headers of dos_api.cu under C++20
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -24,7 +25,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for src in SOURCES:
         obj = os.path.join(HERE, src.replace(".cu", ".o"))
         objs.append(obj)
-        cmd = [nvcc] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(HERE, src), "-o", obj]
+        cmd = [nvcc] + FLAGS + [STD.get(src, "-std=c++17")] + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(HERE, src), "-o", obj]
         procs.append((cmd, subprocess.Popen(cmd)))
     for cmd, p in procs:
         if p.wait() != 0:

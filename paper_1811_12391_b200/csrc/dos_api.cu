@@ -16,7 +16,8 @@
 
 struct Layout {
     size_t phi_u, phi_all, qfix, q, fy, fz, done, queue, items, items_u, mat, dose_acc, sig_t, sig_s, kerma, m2d, d2m, cdd,
-        bm2d, bd2m, signs, errflag, bx, by, bz, phi00_old, conv, um, phi_u_sum, total;
+        bm2d, bd2m, signs, errflag, bx, by, bz, phi00_old, conv, um, phi_u_sum, slot, total;
+    int n_slots;
 };
 
 struct dos_ctx {
@@ -37,7 +38,8 @@ struct dos_ctx {
     std::vector<int> band_lo;    // [G]: lowest g' with a non-zero sigma_s^{g'->g}
     int state;                   // 0 created, 1 uncollided done, 2 solved
     bool can_sum, summed;        // workspace holds the summed-source buffers; the current uncollided state is a sum
-    dos_source src;
+    std::vector<dos_source> srcs;   // sources of the position slots in use
+    int n_slots, active;         // position slots of the workspace; slots the current uncollided state fills (1 unless dos_uncollided_batch)
     bool have_dose_acc;
     bool mat_checked;            // the current material grid has been through validate_material_kernel
     int refl;                    // reflective faces: bit 0 x, 1 y, 2 z (dos_set_boundary); 0 = vacuum
@@ -98,9 +100,13 @@ static void host_ylm(double mu, double eta, double xi, int L, double *y)
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
-static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L, int n_ang, bool summed)
+// Workspace = n_slots "slots" (everything one source position owns: its uncollided fluence, all groups' moments, the
+// sweep's source, face buffers, flags and boundary buffers; slot b starts slot bytes x b further on) followed by what the
+// positions share (work queue and items, material copy, tables, summed-source buffers).
+static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L, int n_ang, int n_slots)
 {
     Layout l;
+    const bool summed = n_slots > 1;
     const size_t nv = (size_t)m->nx * m->ny * m->nz;
     const int MP = dos_mpad(L), per = n_ang / 8;
     const int ntj = (m->ny + DOS_TJ - 1) / DOS_TJ, ntk = (m->nz + DOS_TK - 1) / DOS_TK;
@@ -110,6 +116,7 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     const size_t fz = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TJ;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+    // ---- per slot ----
     l.phi_u = take(sizeof(float) * G * nv);
     l.phi_all = take(sizeof(float) * G * nv * MP);
     l.qfix = take(sizeof(float) * nv * MP);
@@ -117,6 +124,15 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.fy = take(sizeof(float) * fy);
     l.fz = take(sizeof(float) * fz);
     l.done = take(sizeof(int) * (size_t)8 * ntj * ntk * 8);      // FFMA sweep: up to 8 angle parts per (octant, tile)
+    // reflective boundaries (tensor-memory sweep): two halves (previous / current sweep) of the boundary outflow
+    l.bx = take(sizeof(float) * (size_t)2 * 8 * per * m->nz * m->ny);
+    l.by = take(sizeof(float) * (size_t)2 * 8 * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK);
+    l.bz = take(sizeof(float) * (size_t)2 * 8 * ntj * (m->nx + DOS_FACE_PAD) * per * DOS_TJ);
+    l.phi00_old = take(sizeof(float) * nv);                       // tolerance-stopped solve: scalar fluence of the previous iterate
+    l.slot = off;
+    l.n_slots = n_slots;
+    off = l.slot * (size_t)n_slots;
+    // ---- shared ----
     l.queue = take(sizeof(int) * 4);
     l.items = take(sizeof(int) * (size_t)8 * ntj * ntk);
     l.items_u = take(sizeof(int) * (size_t)2 * ntj * ntk);
@@ -132,12 +148,6 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     l.bd2m = take(sizeof(float) * (size_t)2 * NMP * A8);
     l.signs = take(sizeof(unsigned) * (size_t)8 * MP);
     l.errflag = take(sizeof(int) * 4);
-    // reflective boundaries (tensor-memory sweep): two halves (previous / current sweep) of the boundary outflow
-    l.bx = take(sizeof(float) * (size_t)2 * 8 * per * m->nz * m->ny);
-    l.by = take(sizeof(float) * (size_t)2 * 8 * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK);
-    l.bz = take(sizeof(float) * (size_t)2 * 8 * ntj * (m->nx + DOS_FACE_PAD) * per * DOS_TJ);
-    // tolerance-stopped solve: scalar fluence of the previous iterate, two reduction words
-    l.phi00_old = take(sizeof(float) * nv);
     l.conv = take(sizeof(int) * 4);
     // summed-source mode (dos_uncollided_sum): uncollided moments of all positions and their scalar sum
     l.um = summed ? take(sizeof(float) * G * nv * MP) : 0;
@@ -212,7 +222,8 @@ extern "C" dos_status dos_workspace_bytes(const dos_mesh *mesh, const dos_xs *xs
     dos_status s = check_inputs(mesh, xs, quad, P_L);
     if (s != DOS_OK) return s;
     if (n_batch < 1) return fail(nullptr, DOS_ERR_INVALID_ARG, "n_batch must be >= 1");
-    *bytes_out = make_layout(mesh, xs->n_mat, xs->n_group, xs->n_leg, P_L, quad->n_ang, n_batch > 1).total;
+    if (n_batch > 64) return fail(nullptr, DOS_ERR_UNSUPPORTED, "n_batch > 64");
+    *bytes_out = make_layout(mesh, xs->n_mat, xs->n_group, xs->n_leg, P_L, quad->n_ang, n_batch).total;
     return DOS_OK;
 }
 
@@ -249,11 +260,13 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
                 quad->eta[n] != ey || quad->xi[n] != ez || quad->w[n] != quad->w[t])
                 return fail(nullptr, DOS_ERR_INVALID_ARG, "quadrature is not octant-major / octant-symmetric");
         }
-    // a workspace sized with n_batch > 1 also holds the buffers of the summed-source mode
-    Layout lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang, true);
-    const bool can_sum = workspace_bytes >= lay.total;
-    if (!can_sum) lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang, false);
-    if (workspace_bytes < lay.total) return fail(nullptr, DOS_ERR_SHAPE, "workspace too small");
+    // the number of position slots is what the workspace was sized for (dos_workspace_bytes' n_batch): the largest count
+    // whose layout fits; with more than one slot it also holds the buffers of the summed-source mode
+    int n_slots = 0;
+    for (int n = 1; n <= 64 && make_layout(mesh, n_mat, G, n_leg, L, n_ang, n).total <= workspace_bytes; ++n) n_slots = n;
+    if (n_slots < 1) return fail(nullptr, DOS_ERR_SHAPE, "workspace too small");
+    const Layout lay = make_layout(mesh, n_mat, G, n_leg, L, n_ang, n_slots);
+    const bool can_sum = n_slots > 1;
 
     dos_ctx *c = new (std::nothrow) dos_ctx();
     if (!c) return fail(nullptr, DOS_ERR_NOMEM, "out of host memory");
@@ -273,6 +286,8 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->grid = c->grid_u = 0;
     c->mat_checked = false;
     c->refl = 0;
+    c->n_slots = n_slots; c->active = 0;
+    c->srcs.resize(n_slots);
     c->nv = (size_t)mesh->nx * mesh->ny * mesh->nz;
     c->stream = (cudaStream_t)cuda_stream;
     c->d_mat = d_material_ids;
@@ -463,7 +478,7 @@ extern "C" dos_status dos_set_material_host(dos_ctx *c, const uint8_t *h_materia
 }
 
 // mode 0: single source; 1: first source of a sum; 2: further source of a sum
-static dos_status uncollided_impl(dos_ctx *c, const dos_source *source, const float *spectrum, float *d_phi_u_out, int mode)
+static dos_status uncollided_impl(dos_ctx *c, const dos_source *source, const float *spectrum, float *d_phi_u_out, int mode, int slot = 0)
 {
     if (!c || !source || !spectrum) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
     if (mode && !c->can_sum) return fail(c, DOS_ERR_STATE, "the workspace was not sized for the summed-source mode (dos_workspace_bytes with n_batch > 1)");
@@ -494,8 +509,8 @@ static dos_status uncollided_impl(dos_ctx *c, const dos_source *source, const fl
         if (!(spectrum[g] >= 0.f)) return fail(c, DOS_ERR_INVALID_ARG, "spectrum must be >= 0");
         sp.s[g] = (double)spectrum[g];
     }
-    c->src = *source;
-    float *phi_u = (float *)(c->ws + c->lay.phi_u);
+    c->srcs[slot] = *source;
+    float *phi_u = (float *)(c->ws + c->lay.phi_u + (size_t)slot * c->lay.slot);
     prof_begin(c, 1);
     CUDA_TRY(c, dos_launch_raytrace(mesh_dev(c->mesh), source_dev(*source), c->d_mat, c->n_mat, c->G,
                                     (const float *)(c->ws + c->lay.sig_t), sp,
@@ -510,7 +525,22 @@ static dos_status uncollided_impl(dos_ctx *c, const dos_source *source, const fl
     c->summed = mode != 0;
     if (d_phi_u_out)
         CUDA_TRY(c, cudaMemcpyAsync(d_phi_u_out, phi_u, sizeof(float) * c->G * c->nv, cudaMemcpyDeviceToDevice, c->stream));
+    c->active = slot + 1;
     c->state = 1;
+    return DOS_OK;
+}
+
+extern "C" dos_status dos_uncollided_batch(dos_ctx *c, int32_t n_sources, const dos_source *sources, const float *spectrum,
+                                           float *d_phi_u_out)
+{
+    if (!c || !sources) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
+    if (n_sources < 1 || n_sources > c->n_slots)
+        return fail(c, n_sources < 1 ? DOS_ERR_INVALID_ARG : DOS_ERR_STATE,
+                    "dos_uncollided_batch: the workspace was sized for fewer source positions (dos_workspace_bytes' n_batch)");
+    for (int b = 0; b < n_sources; ++b) {
+        dos_status st = uncollided_impl(c, &sources[b], spectrum, d_phi_u_out ? d_phi_u_out + (size_t)b * c->G * c->nv : nullptr, 0, b);
+        if (st != DOS_OK) { c->state = 0; c->active = 0; return st; }
+    }
     return DOS_OK;
 }
 
@@ -542,24 +572,27 @@ static dos_status solve_impl(dos_ctx *c, int32_t n_iter, float tol, int32_t *h_i
     if (c->state < 1) return fail(c, DOS_ERR_STATE, "dos_solve before dos_uncollided");
     if (n_iter < 1) return fail(c, DOS_ERR_INVALID_ARG, "n_iter must be >= 1");
     if (c->refl && !c->umma) return fail(c, DOS_ERR_UNSUPPORTED, "reflective boundaries need the tensor-memory sweep");
+    if (tol >= 0.f && c->active > 1) return fail(c, DOS_ERR_UNSUPPORTED, "dos_solve_tol on a position batch");
+    const int nb = c->active;                     // problems swept together (dos_uncollided_batch), 1 otherwise
+    const size_t slot = c->lay.slot;
     const size_t nvm = c->nv * c->MP;
     float *phi_u = (float *)(c->ws + c->lay.phi_u), *phi_all = (float *)(c->ws + c->lay.phi_all);
     float *qfix = (float *)(c->ws + c->lay.qfix), *q = (float *)(c->ws + c->lay.q);
     const float *sig_s = (const float *)(c->ws + c->lay.sig_s);
     int *done = (int *)(c->ws + c->lay.done), *queue = (int *)(c->ws + c->lay.queue);
     const MeshDev md = mesh_dev(c->mesh);
-    const SourceDev sd = source_dev(c->src);
     Sweep2Args a;                       // FFMA sweep
     a.nx = c->mesh.nx; a.ny = c->mesh.ny; a.nz = c->mesh.nz; a.ntj = c->ntj; a.ntk = c->ntk;
     a.per_oct = c->per_oct / c->asplit; a.per_oct_full = c->per_oct; a.a_split = c->asplit;
-    a.n_items = c->n_items * c->asplit; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = c->n_mat;
+    a.n_items = c->n_items * c->asplit * nb; a.n_batch = nb; a.slot_stride = slot; a.n_warps = c->n_grp; a.n_aux = c->n_aux; a.chunk = c->chunk; a.n_mat = c->n_mat;
     a.items = (const int *)(c->ws + c->lay.items); a.Q = q; a.mat = c->d_mat;
     a.m2d = (const float *)(c->ws + c->lay.m2d); a.d2m = (const float *)(c->ws + c->lay.d2m);
     a.cdd = (const float *)(c->ws + c->lay.cdd);
     a.fy = (float *)(c->ws + c->lay.fy); a.fz = (float *)(c->ws + c->lay.fz); a.done = done; a.queue = queue;
     a.abort_flag = (int *)(c->ws + c->lay.errflag) + 1;
     SweepUArgs u;                       // tensor-memory sweep
-    u.nx = a.nx; u.ny = a.ny; u.nz = a.nz; u.ntj = a.ntj; u.ntk = a.ntk; u.n_items = c->n_items_u; u.per_oct = c->per_oct;
+    u.nx = a.nx; u.ny = a.ny; u.nz = a.nz; u.ntj = a.ntj; u.ntk = a.ntk; u.n_items = c->n_items_u * nb; u.n_batch = nb; u.slot_stride = slot;
+    u.per_oct = c->per_oct;
     u.MP = c->MP; u.chunk = c->chunk; u.n_mat = c->n_mat;
     u.items = (const int *)(c->ws + c->lay.items_u); u.Q = q; u.mat = c->d_mat; u.cdd = a.cdd;
     u.bm2d = (const float *)(c->ws + c->lay.bm2d); u.bd2m = (const float *)(c->ws + c->lay.bd2m);
@@ -576,22 +609,28 @@ static dos_status solve_impl(dos_ctx *c, int32_t n_iter, float tol, int32_t *h_i
     int sweep_no = 0;
     for (int g = 0; g < c->G; ++g) {
         float *phi = phi_all + (size_t)g * nvm;
-        CUDA_TRY(c, dos_launch_group_source(md, sd, c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s, phi_u,
-                                            c->summed ? (const float *)(c->ws + c->lay.um) : nullptr,
-                                            phi_all, qfix, c->stream));
-        c->launches += 1;
+        for (int b = 0; b < nb; ++b) {            // the fixed source depends on the position (Y_lm of the direction from the source)
+            const size_t sh = (size_t)b * slot / sizeof(float);
+            CUDA_TRY(c, dos_launch_group_source(md, source_dev(c->srcs[b]), c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, c->band_lo[g], sig_s,
+                                                phi_u + sh, c->summed ? (const float *)(c->ws + c->lay.um) : nullptr, phi_all + sh,
+                                                qfix + sh, c->stream));
+            c->launches += 1;
+        }
         a.phi = u.phi = phi;
         a.sig_t = u.sig_t = (const float *)(c->ws + c->lay.sig_t) + (size_t)g * c->n_mat;
         if (c->refl) {
             // every group starts from zero boundary inflow (the lagged reflective condition of the first sweep)
-            CUDA_TRY(c, cudaMemsetAsync(bx, 0, sizeof(float) * 2 * bxh, c->stream));
-            CUDA_TRY(c, cudaMemsetAsync(by, 0, sizeof(float) * 2 * byh, c->stream));
-            CUDA_TRY(c, cudaMemsetAsync(bz, 0, sizeof(float) * 2 * bzh, c->stream));
+            for (int b = 0; b < nb; ++b) {
+                const size_t sh = (size_t)b * slot / sizeof(float);
+                CUDA_TRY(c, cudaMemsetAsync(bx + sh, 0, sizeof(float) * 2 * bxh, c->stream));
+                CUDA_TRY(c, cudaMemsetAsync(by + sh, 0, sizeof(float) * 2 * byh, c->stream));
+                CUDA_TRY(c, cudaMemsetAsync(bz + sh, 0, sizeof(float) * 2 * bzh, c->stream));
+            }
         }
         int it = 0;
         for (; it < n_iter; ++it) {
             CUDA_TRY(c, dos_launch_source_update(c->nv, c->d_mat, c->n_mat, c->G, c->n_leg, c->L, g, sig_s, qfix, phi, q, it == 0,
-                                                 done, n_flags, queue, phi00_old, c->stream));
+                                                 done, n_flags, queue, phi00_old, nb, slot, c->stream));
             const int cur = sweep_no & 1, prv = cur ^ 1;
             u.bx_in = bx + prv * bxh; u.bx_out = bx + cur * bxh;
             u.by_in = by + prv * byh; u.by_out = by + cur * byh;
@@ -662,9 +701,13 @@ extern "C" dos_status dos_fluence(dos_ctx *c, float *d_phi_collided, float *d_ph
 {
     if (!c) return fail(c, DOS_ERR_INVALID_ARG, "null context");
     if (c->state < 2) return fail(c, DOS_ERR_STATE, "dos_fluence before dos_solve");
-    CUDA_TRY(c, dos_launch_fluence(c->nv, c->G, c->MP, (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u)),
-                                   (const float *)(c->ws + c->lay.phi_all), d_phi_collided, d_phi_total, c->stream));
-    c->launches += 1;
+    for (int b = 0; b < c->active; ++b) {         // a position batch fills [n_sources][G][nz][ny][nx]
+        const size_t sh = (size_t)b * c->lay.slot, out = (size_t)b * c->G * c->nv;
+        CUDA_TRY(c, dos_launch_fluence(c->nv, c->G, c->MP, (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u + sh)),
+                                       (const float *)(c->ws + c->lay.phi_all + sh), d_phi_collided ? d_phi_collided + out : nullptr,
+                                       d_phi_total ? d_phi_total + out : nullptr, c->stream));
+        c->launches += 1;
+    }
     return DOS_OK;
 }
 
@@ -672,10 +715,13 @@ extern "C" dos_status dos_dose(dos_ctx *c, float *d_dose, int32_t accumulate)
 {
     if (!c || !d_dose) return fail(c, DOS_ERR_INVALID_ARG, "null argument");
     if (c->state < 2) return fail(c, DOS_ERR_STATE, "dos_dose before dos_solve");
-    CUDA_TRY(c, dos_launch_dose(c->nv, c->d_mat, c->n_mat, c->G, c->MP, (const float *)(c->ws + c->lay.kerma),
-                                (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u)), (const float *)(c->ws + c->lay.phi_all), d_dose,
-                                accumulate, c->stream));
-    c->launches += 1;
+    for (int b = 0; b < c->active; ++b) {         // a position batch: the doses of its positions are summed (a9)
+        const size_t sh = (size_t)b * c->lay.slot;
+        CUDA_TRY(c, dos_launch_dose(c->nv, c->d_mat, c->n_mat, c->G, c->MP, (const float *)(c->ws + c->lay.kerma),
+                                    (const float *)(c->ws + (c->summed ? c->lay.phi_u_sum : c->lay.phi_u + sh)),
+                                    (const float *)(c->ws + c->lay.phi_all + sh), d_dose, accumulate || b > 0, c->stream));
+        c->launches += 1;
+    }
     return DOS_OK;
 }
 

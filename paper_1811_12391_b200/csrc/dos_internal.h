@@ -51,6 +51,11 @@ struct Sweep2Args {
     int *done;               // [n_items (by id)] steps finished and published
     int *queue;              // work-queue head
     int *abort_flag;         // set by the watchdog; every waiting CTA then stops waiting
+    // position batch: n_batch independent problems on the same mesh / tables in one launch. Work item
+    // i is tile item i / n_batch of problem i % n_batch; Q, phi, fy, fz, done of problem b sit slot_stride BYTES x b
+    // behind the pointers above.
+    int n_batch;
+    size_t slot_stride;
 };
 
 cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ang_per_warp, int grid, int two_per_sm, cudaStream_t s);
@@ -91,6 +96,10 @@ struct SweepUArgs {
     const float *bz_in;      // [8][ntj][nx + PAD][A][TJ]
     float *bz_out;
     int refl;
+    // position batch: work item i is tile item i / n_batch of problem i % n_batch; Q, phi, fy, fz, done
+    // and the boundary buffers of problem b sit slot_stride BYTES x b behind the pointers above.
+    int n_batch;
+    size_t slot_stride;
 };
 int dos_sweep_umma_supported(int per_oct, int L);
 cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int *grid_out);

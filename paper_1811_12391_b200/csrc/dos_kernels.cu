@@ -221,11 +221,20 @@ __global__ void __launch_bounds__(256) source_update_kernel(size_t nv, int MV, i
                                                             int n_mat, int G, int n_leg, int g, const float *__restrict__ sig_s,
                                                             const float4 *__restrict__ qfix, float4 *__restrict__ phi,
                                                             float4 *__restrict__ q, int first, int *done, int n_flags,
-                                                            int *queue, float *__restrict__ phi00_old)
+                                                            int *queue, float *__restrict__ phi00_old, size_t slot_stride)
 {
+    // blockIdx.y = problem of the position batch: its buffers sit slot_stride bytes x blockIdx.y further on
+    {
+        const size_t sh = (size_t)blockIdx.y * slot_stride;
+        qfix = reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(qfix) + sh);
+        phi = reinterpret_cast<float4 *>(reinterpret_cast<char *>(phi) + sh);
+        q = reinterpret_cast<float4 *>(reinterpret_cast<char *>(q) + sh);
+        done = reinterpret_cast<int *>(reinterpret_cast<char *>(done) + sh);
+        if (phi00_old) phi00_old = reinterpret_cast<float *>(reinterpret_cast<char *>(phi00_old) + sh);
+    }
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t < (size_t)n_flags) done[t] = 0;
-    if (t == 0) *queue = 0;
+    if (t == 0 && blockIdx.y == 0) *queue = 0;
     if (t >= nv * MV) return;
     const size_t cell = t / MV;
     const int v = (int)(t - cell * MV);
@@ -296,14 +305,15 @@ cudaError_t dos_launch_group_source(const MeshDev &m, const SourceDev &s, const 
 
 cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int n_mat, int G, int n_leg, int L, int g, const float *sig_s,
                                      const float *qfix, float *phi, float *q, int first, int *done, int n_flags,
-                                     int *queue, float *phi00_old, cudaStream_t st)
+                                     int *queue, float *phi00_old, int n_batch, size_t slot_stride, cudaStream_t st)
 {
     const int M = (L + 1) * (L + 1), MV = dos_mpad(L) / 4;
     size_t n = nv * MV;
     if ((size_t)n_flags > n) n = (size_t)n_flags;
     const unsigned grid = (unsigned)((n + 255) / 256);
-    source_update_kernel<<<grid, 256, 0, st>>>(nv, MV, M, mat, n_mat, G, n_leg, g, sig_s, (const float4 *)qfix, (float4 *)phi,
-                                               (float4 *)q, first, done, n_flags, queue, phi00_old);
+    source_update_kernel<<<dim3(grid, (unsigned)n_batch), 256, 0, st>>>(nv, MV, M, mat, n_mat, G, n_leg, g, sig_s, (const float4 *)qfix,
+                                                                        (float4 *)phi, (float4 *)q, first, done, n_flags, queue, phi00_old,
+                                                                        slot_stride);
     return cudaGetLastError();
 }
 

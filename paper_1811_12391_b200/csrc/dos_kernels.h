@@ -40,7 +40,8 @@ cudaError_t dos_launch_um_accumulate(const MeshDev &m, const SourceDev &s, int G
 // flags (n_flags ints at `done`) and its queue head.
 cudaError_t dos_launch_source_update(size_t nv, const uint8_t *mat, int n_mat, int G, int n_leg, int L, int g,
                                      const float *sig_s, const float *qfix, float *phi, float *q, int first,
-                                     int *done, int n_flags, int *queue, float *phi00_old /* or null */, cudaStream_t st);
+                                     int *done, int n_flags, int *queue, float *phi00_old /* or null */, int n_batch,
+                                     size_t slot_stride /* bytes between the problems of a position batch */, cudaStream_t st);
 // out2[0] = max |phi00 - phi00_old|, out2[1] = max |phi00| over the cells, as float bit patterns
 cudaError_t dos_launch_conv(size_t nv, int MP, const float *phi, const float *phi00_old, int *out2, cudaStream_t st);
 

@@ -203,8 +203,9 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
 //   service warp   NW + NX + 1    global hand-off flags (never joins the per-step barrier)
 // TMAX = CTA size bound for the register budget.
 template <int MP, int AG, int TMAX, int MINB>
-__global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
+__global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
 {
+    Sweep2Args p = p0;       // Q, phi, fy, fz, done are re-pointed at the item's problem of the batch
     constexpr int MV = MP / 4, MPS = mps_of(MP);
     extern __shared__ float4 smem4[];
     const int A = p.per_oct, NW = p.n_warps, NX = p.n_aux;
@@ -237,8 +238,16 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p)
         __syncthreads();                              // previous item finished with the staging buffers
         if (tid == 0) s_item = atomicAdd(p.queue, 1);
         __syncthreads();
-        const int item = s_item;
-        if (item >= p.n_items) break;
+        if (s_item >= p.n_items) break;
+        const int item = s_item / p.n_batch;
+        {
+            const size_t sh = (size_t)(s_item - item * p.n_batch) * p.slot_stride;
+            p.Q = reinterpret_cast<const float *>(reinterpret_cast<const char *>(p0.Q) + sh);
+            p.phi = reinterpret_cast<float *>(reinterpret_cast<char *>(p0.phi) + sh);
+            p.fy = reinterpret_cast<float *>(reinterpret_cast<char *>(p0.fy) + sh);
+            p.fz = reinterpret_cast<float *>(reinterpret_cast<char *>(p0.fz) + sh);
+            p.done = reinterpret_cast<int *>(reinterpret_cast<char *>(p0.done) + sh);
+        }
         const int tile_item = item / p.a_split, part = item - tile_item * p.a_split;
         const int packed = p.items[tile_item];
         ItemGeom g;

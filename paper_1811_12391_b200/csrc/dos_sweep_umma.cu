@@ -150,8 +150,9 @@ __device__ __forceinline__ void split_piece(const float4 *src, const unsigned *s
 //   4 NG        M2D issuer (one elected lane)      4 NG + 1   D2M issuer
 //   4 NG + 2    feeder (tile-inflow faces)         4 NG + 3   service (global hand-off flags)
 template <int AG, int NG>
-__global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const SweepUArgs p)
+__global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const SweepUArgs p0)
 {
+    SweepUArgs p = p0;       // Q, phi, face and boundary buffers, done are re-pointed at the item's problem of the batch
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int A = p.per_oct, MP = p.MP, KP = (MP + 7) & ~7, NCH = KP / 4, A8 = (A + 7) & ~7, NAP = (A + 15) & ~15, NMP = (MP + 15) & ~15;
     constexpr int NCW = 4 * NG;
@@ -239,14 +240,21 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
         if (tid == 0) s_item = atomicAdd(p.queue, 1);
         if (tid < NCW) s_prog[tid] = 0;
         __syncthreads();
-        const int item = s_item;
-        if (item >= p.n_items) return false;
+        if (s_item >= p.n_items) return false;
+        const int item = s_item / p.n_batch;
+        {
+            const size_t sh = (size_t)(s_item - item * p.n_batch) * p.slot_stride;
+            auto mv = [sh](auto *ptr) { return reinterpret_cast<decltype(ptr)>(reinterpret_cast<size_t>(ptr) + sh); };
+            p.Q = mv(p0.Q); p.phi = mv(p0.phi); p.fy = mv(p0.fy); p.fz = mv(p0.fz); p.done = mv(p0.done);
+            p.bx_in = mv(p0.bx_in); p.bx_out = mv(p0.bx_out); p.by_in = mv(p0.by_in); p.by_out = mv(p0.by_out);
+            p.bz_in = mv(p0.bz_in); p.bz_out = mv(p0.bz_out);
+        }
         const int packed = p.items[item];
         quad = packed & 7; tj = (packed >> 3) & 0x3FFF; tk = packed >> 17;
         fid = (quad * p.ntk + tk) * p.ntj + tj;      // hand-off flag of this (quad, tile)
         has_y = tj > 0 || (p.refl & 2); has_z = tk > 0 || (p.refl & 4);      // there is y / z inflow to stage (else vacuum)
 #if DOS_UMMA_TRACE
-        trace_on = item == 601;
+        trace_on = s_item == 601;
 #endif
         return true;
     };

@@ -20,7 +20,7 @@ DOS_OK = 0
 STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_ERR_STATE", -4: "DOS_ERR_NOMEM",
           -5: "DOS_ERR_CUDA", -6: "DOS_ERR_UNSUPPORTED"}
 
-EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_sum",
+EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_batch", "dos_uncollided_sum",
            "dos_uncollided_total", "dos_solve", "dos_solve_tol", "dos_set_boundary", "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option",
            "dos_profile", "dos_profile_reset", "dos_destroy", "dos_last_error"]
 
@@ -59,6 +59,8 @@ _lib.dos_set_material_host.restype = C.c_int
 _lib.dos_set_material_host.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dos_uncollided.restype = C.c_int
 _lib.dos_uncollided.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.dos_uncollided_batch.restype = C.c_int
+_lib.dos_uncollided_batch.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.dos_uncollided_sum.restype = C.c_int
 _lib.dos_uncollided_sum.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
 _lib.dos_solve.restype = C.c_int
@@ -157,6 +159,7 @@ class Context:
         self.mesh = dict(mesh)
         self.device = torch.device(device)
         self.G = int(np.asarray(sigma_t).shape[1])
+        self.n_batch = int(n_batch)
         self.shape = (mesh["nz"], mesh["ny"], mesh["nx"])
         self._tables = _Tables(sigma_t, sigma_s, kerma, quad)
         nbytes = dos_workspace_bytes(mesh, sigma_t, sigma_s, kerma, quad, P_L, n_batch)
@@ -190,6 +193,13 @@ class Context:
         sp = _f32(spectrum)
         ptr = phi_u_out.data_ptr() if phi_u_out is not None else None
         self._check(_lib.dos_uncollided(self.handle, C.byref(src), sp.ctypes.data, ptr))
+
+    def dos_uncollided_batch(self, sources, spectrum, phi_u_out=None):
+        """Up to n_batch source positions at once; the following dos_solve sweeps them in the same launches."""
+        arr = (dos_source * len(sources))(*[_source_struct(s) for s in sources])
+        sp = _f32(spectrum)
+        ptr = phi_u_out.data_ptr() if phi_u_out is not None else None
+        self._check(_lib.dos_uncollided_batch(self.handle, len(sources), arr, sp.ctypes.data, ptr))
 
     def dos_uncollided_sum(self, source, spectrum, first, phi_u_out=None):
         src = _source_struct(source)

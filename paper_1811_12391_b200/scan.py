@@ -16,13 +16,19 @@ def shard_positions(n_pos: int, rank: int, world: int):
 
 
 def run_scan(ctx, problem, positions, dose, n_iter=None):
-    """Runs the hot path for each listed position on `ctx`, summing the dose maps into `dose` (device
-    tensor [nz][ny][nx]); with no positions the map is zeroed. Only enqueues work."""
+    """Runs the hot path for the listed positions on `ctx`, summing the dose maps into `dose` (device tensor
+    [nz][ny][nx]); with no positions the map is zeroed. Positions go through the library ctx.n_batch at a time
+    (dos_uncollided_batch: one set of sweep launches serves the whole batch). Only enqueues work."""
     n_iter = problem["n_iter"] if n_iter is None else n_iter
     if not positions:
         dose.zero_()
-    for n, s in enumerate(positions):
-        ctx.dos_uncollided(problem["sources"][s], problem["spectrum"])
+    nb = max(1, int(getattr(ctx, "n_batch", 1)))
+    for n in range(0, len(positions), nb):
+        chunk = [problem["sources"][s] for s in positions[n:n + nb]]
+        if len(chunk) == 1:
+            ctx.dos_uncollided(chunk[0], problem["spectrum"])
+        else:
+            ctx.dos_uncollided_batch(chunk, problem["spectrum"])
         ctx.dos_solve(n_iter)
         ctx.dos_dose(dose, accumulate=(n > 0))
     return dose

@@ -212,6 +212,60 @@ def test_config5_full_mesh_properties(dos, orc):
     ctx.close()
 
 
+# ------------------------------------------------- position batch --
+def test_position_batch_equals_separate_solves(dos, orc):
+    """dos_uncollided_batch + one dos_solve for several source positions: per-position fluences equal those of separate
+    solves (same kernels, same arithmetic; only the order of the moment reductions may differ) and match the oracle; the
+    dose is the sum over the positions (a9); both sweep kernels; a batch smaller than the slot count; state machine."""
+    import torch
+    from paper_1811_12391_b200 import scan
+    for name, ov, opts in (("config4", dict(nx=30, ny=27, nz=7, voxel=1.3, n_group=4, n_iter=3, n_pos=5), {}),
+                           ("config3", dict(nx=18, ny=11, nz=9, voxel=2.0, n_group=2, n_iter=3), {}),
+                           ("config4", dict(nx=30, ny=27, nz=7, voxel=1.3, n_group=3, n_iter=3, n_pos=5), {"sweep_contraction": 2})):
+        p = _make(name, **ov)
+        if len(p["sources"]) == 1:      # config 3: three positions around the cylinder
+            from paper_1811_12391_b200.inputs import scan_source
+            p["sources"] = [scan_source(th) for th in (0.5 * math.pi, 1.1, 4.0)]
+        pos = [0, 2, 1] if len(p["sources"]) == 3 else [0, 3, 4]
+        ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"], n_batch=4)
+        for k, v in opts.items():
+            ctx.dos_set_option(k, v)
+        G = p["n_group"]
+        pu = torch.empty((3, G) + ctx.shape, dtype=torch.float32, device=ctx.device)
+        pc, pt = torch.empty_like(pu), torch.empty_like(pu)
+        d = ctx.new_field(groups=False)
+        ctx.dos_uncollided_batch([p["sources"][s] for s in pos], p["spectrum"], pu)
+        ctx.dos_solve(p["n_iter"])
+        ctx.dos_fluence(pc, pt)
+        ctx.dos_dose(d, False)
+        ctx.dos_check()
+        ref_dose = 0.0
+        for b, s_ in enumerate(pos):
+            ref = orc.run_problem(p, source_index=s_)
+            out = {"phi_u": pu[b].cpu().numpy(), "phi_c": pc[b].cpu().numpy(), "phi_total": pt[b].cpu().numpy(), "dose": ref["dose"]}
+            assert_problem_parity(out, ref, f"{name} batch slot {b}")
+            ref_dose = ref_dose + ref["dose"]
+            one = dos.run_problem(p, source_index=s_, ctx=None)      # a separate solve on a fresh single-slot context
+            assert np.array_equal(one["phi_u"], out["phi_u"])
+            assert np.abs(one["phi_c"] - out["phi_c"]).max() <= 2e-6 * np.abs(one["phi_c"]).max()
+        assert_dose_parity(d.cpu().numpy(), ref_dose, "batch dose = sum over positions")
+        # the same context serves a smaller batch and a single position afterwards
+        ctx.dos_uncollided_batch([p["sources"][pos[1]]], p["spectrum"])
+        ctx.dos_solve(p["n_iter"])
+        ctx.dos_dose(d, False)
+        assert_dose_parity(d.cpu().numpy(), orc.run_problem(p, source_index=pos[1])["dose"], "batch of one")
+        with pytest.raises(dos.DosError) as e:
+            ctx.dos_uncollided_batch([p["sources"][0]] * 5, p["spectrum"])
+        assert e.value.status == -3
+        # scan.run_scan drives the batch path: 5 (or 3) positions through 4 slots
+        all_pos = list(range(len(p["sources"])))
+        scan.run_scan(ctx, p, all_pos, d)
+        ctx.dos_check()
+        tot = sum(orc.run_problem(p, source_index=s_)["dose"] for s_ in all_pos)
+        assert_dose_parity(d.cpu().numpy(), tot, "run_scan through the batch path")
+        ctx.close()
+
+
 # ------------------------------------------------- SURVEY 8(f) N3: reflective boundaries, stopping rule --
 def test_reflective_boundaries_parity_and_balance(dos, orc):
     """dos_set_boundary (PAPER.md:41 states vacuum; north_star check 2 needs reflective faces). (a) GPU vs the oracle's
