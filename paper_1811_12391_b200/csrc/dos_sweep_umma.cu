@@ -94,10 +94,13 @@ __device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_
 {
     if (mbar_try_wait(bar, parity)) return;
 #pragma unroll 1
-    for (int spins = 0; spins < WAIT_LIMIT; ++spins) {
-        __nanosleep(sleep_ns);
-        if (mbar_try_wait(bar, parity)) return;
-        if ((spins & 1023) == 1023 && *(volatile int *)s_abort) return;
+    for (int outer = 0; outer < WAIT_LIMIT / 1024; ++outer) {
+#pragma unroll 1
+        for (int spins = 0; spins < 1024; ++spins) {      // the poll itself: sleep, try, branch
+            __nanosleep(sleep_ns);
+            if (mbar_try_wait(bar, parity)) return;
+        }
+        if (*(volatile int *)s_abort) return;
     }
     *(volatile int *)s_abort = 1;
     atomicExch(g_abort, 1);
@@ -149,10 +152,13 @@ __device__ __forceinline__ void split_piece(const float4 *src, const unsigned *s
 //   [0, 4 NG)   compute: octant q = warp % 4, angle group g = warp / 4 (also: its share of staging, split, read-back)
 //   4 NG        M2D issuer (one elected lane)      4 NG + 1   D2M issuer
 //   4 NG + 2    feeder (tile-inflow faces)         4 NG + 3   service (global hand-off flags)
-template <int AG, int NG>
-__global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const SweepUArgs p0)
+// REFL: the variant with reflective mesh faces (lagged boundary buffers); the vacuum-only variant carries none of it.
+template <int AG, int NG, bool REFL>
+__global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const SweepUArgs p)
 {
-    SweepUArgs p = p0;       // Q, phi, face and boundary buffers, done are re-pointed at the item's problem of the batch
+    const int refl = REFL ? p.refl : 0;
+    size_t sh = 0;           // byte offset of the item's problem of the position batch: Q, phi, faces, boundaries, done
+    auto mv = [&sh](auto *ptr) { return reinterpret_cast<decltype(ptr)>(reinterpret_cast<size_t>(ptr) + sh); };
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int A = p.per_oct, MP = p.MP, KP = (MP + 7) & ~7, NCH = KP / 4, A8 = (A + 7) & ~7, NAP = (A + 15) & ~15, NMP = (MP + 15) & ~15;
     constexpr int NCW = 4 * NG;
@@ -169,6 +175,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
     float *s_rden = reinterpret_cast<float *>(carve((size_t)p.n_mat * A * 4));                  // [n_mat][A]
     float *s_sig = reinterpret_cast<float *>(carve((size_t)p.n_mat * 4));
     unsigned *s_sign = reinterpret_cast<unsigned *>(carve((size_t)8 * MP * 4));                 // [8 octants][MP] 0 or 0x80000000
+    float *s_zero = reinterpret_cast<float *>(carve((size_t)A * DOS_TJ * 4));                   // vacuum inflow: [A][TJ] zeros
     uint64_t *bars = reinterpret_cast<uint64_t *>(carve(64 * 8));
     int *s_prog = reinterpret_cast<int *>(carve(32 * 4));                                       // [NCW] steps finished per compute warp
     uint64_t *raw_full = bars;            // [RAW][4 octants]
@@ -197,6 +204,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
     for (int i = tid; i < p.n_mat * A; i += blockDim.x) s_rden[i] = 1.f / (p.sig_t[i / A] + p.cdd[(i % A) * 4 + 3]);
     for (int i = tid; i < p.n_mat; i += blockDim.x) s_sig[i] = p.sig_t[i];
     for (int i = tid; i < 8 * MP; i += blockDim.x) s_sign[i] = p.signs[i];
+    for (int i = tid; i < A * DOS_TJ; i += blockDim.x) s_zero[i] = 0.f;
     if (tid == 0) {
         for (int i = 0; i < 16; ++i) mbar_init(&raw_full[i], 32 * NG);      // one cp.async arrival per thread of the octant's warps
         for (int i = 0; i < ASL; ++i) { mbar_init(&a_full[i], NCW); mbar_init(&a_empty[i], 1); }
@@ -242,17 +250,11 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
         __syncthreads();
         if (s_item >= p.n_items) return false;
         const int item = s_item / p.n_batch;
-        {
-            const size_t sh = (size_t)(s_item - item * p.n_batch) * p.slot_stride;
-            auto mv = [sh](auto *ptr) { return reinterpret_cast<decltype(ptr)>(reinterpret_cast<size_t>(ptr) + sh); };
-            p.Q = mv(p0.Q); p.phi = mv(p0.phi); p.fy = mv(p0.fy); p.fz = mv(p0.fz); p.done = mv(p0.done);
-            p.bx_in = mv(p0.bx_in); p.bx_out = mv(p0.bx_out); p.by_in = mv(p0.by_in); p.by_out = mv(p0.by_out);
-            p.bz_in = mv(p0.bz_in); p.bz_out = mv(p0.bz_out);
-        }
+        sh = (size_t)(s_item - item * p.n_batch) * p.slot_stride;
         const int packed = p.items[item];
         quad = packed & 7; tj = (packed >> 3) & 0x3FFF; tk = packed >> 17;
         fid = (quad * p.ntk + tk) * p.ntj + tj;      // hand-off flag of this (quad, tile)
-        has_y = tj > 0 || (p.refl & 2); has_z = tk > 0 || (p.refl & 4);      // there is y / z inflow to stage (else vacuum)
+        has_y = tj > 0 || (refl & 2); has_z = tk > 0 || (refl & 4);      // there is y / z inflow to stage (else vacuum)
 #if DOS_UMMA_TRACE
         trace_on = s_item == 601;
 #endif
@@ -263,8 +265,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
         while (next_item()) {
             // ------- service warp: publishes this item's progress, follows the two upwind items' progress -------
             const bool up_tile_y = tj > 0, up_tile_z = tk > 0;       // boundary inflow (reflective) needs no hand-off
-            const int *up_y = p.done + (up_tile_y ? fid - 1 : fid), *up_z = p.done + (up_tile_z ? fid - p.ntj : fid);
-            int *my_flag = p.done + fid;
+            int *done = mv(p.done);
+            const int *up_y = done + (up_tile_y ? fid - 1 : fid), *up_z = done + (up_tile_z ? fid - p.ntj : fid);
+            int *my_flag = done + fid;
             int avail_y = up_tile_y ? 0 : BIG, avail_z = up_tile_z ? 0 : BIG;
             if (lane == 0) s_allowed = (up_tile_y || up_tile_z) ? -1 : BIG;
             __syncthreads();                          // S2
@@ -314,8 +317,8 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 const bool mine = lane < 8 && (which == 0 ? has_y : has_z);
                 // upwind tile's face buffer -- or, on a reflective mesh boundary, what the mirror octant's last tile
                 // wrote there in the previous sweep (same layout: the boundary is a virtual upwind tile)
-                const float *src = which == 0 ? (tj > 0 ? p.fy + (size_t)(oid - 1) * fstride_y : p.by_in + (size_t)((oo ^ 2) * p.ntk + tk) * fstride_y)
-                                              : (tk > 0 ? p.fz + (size_t)(oid - p.ntj) * fstride_z : p.bz_in + (size_t)((oo ^ 4) * p.ntj + tj) * fstride_z);
+                const float *src = mv(which == 0 ? (tj > 0 ? p.fy + (size_t)(oid - 1) * fstride_y : p.by_in + (size_t)((oo ^ 2) * p.ntk + tk) * fstride_y)
+                                                 : (tk > 0 ? p.fz + (size_t)(oid - p.ntj) * fstride_z : p.bz_in + (size_t)((oo ^ 4) * p.ntj + tj) * fstride_z));
                 const int blk = which == 0 ? A * DOS_TK : A * DOS_TJ;                  // floats per step
                 float *dst0 = which == 0 ? s_finy + qq * blk : s_finz + qq * blk;
                 const unsigned bytes_all = (unsigned)((has_y ? 4 * A * DOS_TK : 0) + (has_z ? 4 * A * DOS_TJ : 0)) * 4u;
@@ -426,20 +429,20 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             // lane (ny - 1) % 8 / (nz - 1) % 4) to the reflective boundary buffer, or nowhere (vacuum)
             const bool last_tj = tj == p.ntj - 1, last_tk = tk == p.ntk - 1;
             const int jst = last_tj ? (p.ny - 1) % DOS_TJ : DOS_TJ - 1, kst = last_tk ? (p.nz - 1) % DOS_TK : DOS_TK - 1;
-            const bool store_y = g.valid && jj == jst && (!last_tj || (p.refl & 2));
-            const bool store_z = g.valid && kk == kst && (!last_tk || (p.refl & 4));
+            const bool store_y = g.valid && jj == jst && (!last_tj || (refl & 2));
+            const bool store_z = g.valid && kk == kst && (!last_tk || (refl & 4));
             const int oid = (o * p.ntk + tk) * p.ntj + tj;
-            float *fy_st = (last_tj ? p.by_out + (size_t)(o * p.ntk + tk) * fstride_y : p.fy + (size_t)oid * fstride_y) + kk +
+            float *fy_st = mv((REFL && last_tj) ? p.by_out + (size_t)(o * p.ntk + tk) * fstride_y : p.fy + (size_t)oid * fstride_y) + kk +
                            ((long long)(-jst) * A + a0) * DOS_TK;
-            float *fz_st = (last_tk ? p.bz_out + (size_t)(o * p.ntj + tj) * fstride_z : p.fz + (size_t)oid * fstride_z) + jj +
+            float *fz_st = mv((REFL && last_tk) ? p.bz_out + (size_t)(o * p.ntj + tj) * fstride_z : p.fz + (size_t)oid * fstride_z) + jj +
                            ((long long)(-kst) * A + a0) * DOS_TJ;
             const int fy_inc = A * DOS_TK, fz_inc = A * DOS_TJ;
-            const float *finy = s_finy + (q * A + a0) * DOS_TK + kk, *finz = s_finz + (q * A + a0) * DOS_TJ + jj;
+            const float *finy0 = s_finy + (q * A + a0) * DOS_TK + kk, *finz0 = s_finz + (q * A + a0) * DOS_TJ + jj;
             const uint8_t *mat_p = p.mat + g.cbase;
             const int istep = g.istep, t_lo = g.t_lo;
             const long long cinc = (long long)istep * MP;                // floats between this lane's consecutive cells
-            const float *qsrc = p.Q + g.cbase * MP;
-            float *phi_base = p.phi + g.cbase * MP;
+            const float *qsrc = mv(p.Q) + g.cbase * MP;
+            float *phi_base = mv(p.phi) + g.cbase * MP;
             const unsigned *sgn = s_sign + o * MP;
             const int nq = MP / 4;                                       // 16-byte pieces of a row; this warp takes grp, grp + NG, ...
             __syncthreads();                          // S2
@@ -500,14 +503,11 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             const int jp_ = tj * DOS_TJ + jj, kp_ = tk * DOS_TK + kk;
             const int jg = (o & 2) ? p.ny - 1 - jp_ : jp_, kg = (o & 4) ? p.nz - 1 - kp_ : kp_;
             const size_t bxi = g.valid ? (size_t)kg * p.ny + jg : 0, bxs = (size_t)p.nz * p.ny;
-            const bool refl_x = (p.refl & 1) && g.valid;
+            const bool refl_x = (refl & 1) && g.valid;
             const int t_last = g.valid ? t_lo + nx - 1 : -1;
             float px[AG], oy[AG], oz[AG];
 #pragma unroll
-            for (int r = 0; r < AG; ++r) {
-                px[r] = refl_x ? __ldcg(p.bx_in + ((size_t)(o ^ 1) * A + a0 + r) * bxs + bxi) : 0.f;
-                oy[r] = oz[r] = 0.f;
-            }
+            for (int r = 0; r < AG; ++r) px[r] = oy[r] = oz[r] = 0.f;
             auto mat_of = [&](int s) -> int { return ((unsigned)(s - t_lo) < (unsigned)nx) ? min((int)__ldg(mat_p + (long long)istep * s), p.n_mat - 1) : 0; };
             int m_cur = mat_of(0), m_nxt = mat_of(1);
             for (int s = 0; s < LA && s < T; ++s) stage(s);
@@ -531,7 +531,17 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 const int fslot = (int)(fs % RFU) * 4 * A;
                 const float *rden = s_rden + m0 * A + a0;
                 const float sig0 = s_sig[m0];
-                const bool last_x = refl_x && t == t_last;
+                if (t == t_lo) {                      // the lane's first cell: seed the x face with the column's inflow
+#pragma unroll
+                    for (int r = 0; r < AG; ++r) {
+                        px[r] = 0.f;
+                        if constexpr (REFL)
+                            if (refl_x) px[r] = __ldcg(mv(p.bx_in) + ((size_t)(o ^ 1) * A + a0 + r) * bxs + bxi);
+                    }
+                }
+                const bool last_x = REFL && refl_x && t == t_last;
+                const bool st_y = store_y && act, st_z = store_z && act;
+                const float *finy = has_y ? finy0 + fslot * DOS_TK : s_zero, *finz = has_z ? finz0 + fslot * DOS_TJ : s_zero;
                 const unsigned tq = tm_dq + lane_base + (gs % DQS) * NAP + a0;            // D_q columns of this warp's angles
                 const unsigned tp = tm_psi + lane_base + (gs % PSL) * 2 * A8 + a0;        // psi operand columns (hi; lo at + A8)
                 // The AG angles go in chunks of CH. Inside a chunk everything is straight-line code (selects, no branches),
@@ -542,20 +552,26 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 // would pin it in the next pass anyway. A pass with nothing new to pin reproduces its input.
                 // Each chunk reads its columns of the discrete source from tensor memory and writes its psi_c (TF32
                 // hi + lo) back as the D2M's A operand, so no per-angle array outlives a chunk except the 3 face fluxes.
-                constexpr int CH = AG <= 4 ? AG : (AG % 3 == 0 ? 3 : 4);
+#ifndef DOS_UMMA_CH
+#define DOS_UMMA_CH 4
+#endif
+                constexpr int CH = AG <= DOS_UMMA_CH ? AG : (AG % DOS_UMMA_CH == 0 ? DOS_UMMA_CH : (AG % 3 == 0 ? 3 : 4));
                 auto chunk = [&]<int C0>() {
                     constexpr int N = AG - C0 < CH ? AG - C0 : CH;
                     float qd[N], ix[N], yi[N], zi[N], ox[N], oyr[N], ozr[N], pc[N];
                     tmem_ld_n<N>(tq + C0, qd);
                     tmem_wait_ld();
-                    bool any = false;
+                    if constexpr (C0 == 0) TRACE(3);
+                    unsigned negm = 0;                // bit e: angle e of the chunk has a negative outflow in this (active) lane
 #pragma unroll
                     for (int e = 0; e < N; ++e) {
                         const int r = C0 + e;
+                        // y / z inflow: the neighbouring lane's outflow of the previous step; lanes on the tile's inflow edge
+                        // take the staged face instead (a zero block stands in for vacuum)
                         float yin = __shfl_up_sync(0xffffffffu, oy[r], 1);
                         float zin = __shfl_up_sync(0xffffffffu, oz[r], DOS_TJ);
-                        if (in_y) yin = has_y ? finy[fslot * DOS_TK + r * DOS_TK] : 0.f;        // tile inflow or vacuum
-                        if (in_z) zin = has_z ? finz[fslot * DOS_TJ + r * DOS_TJ] : 0.f;
+                        if (in_y) yin = finy[r * DOS_TK];
+                        if (in_z) zin = finz[r * DOS_TJ];
                         const float4 cc = cdd4[r];
                         ix[e] = px[r];
                         yi[e] = yin; zi[e] = zin;
@@ -563,45 +579,53 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                         const float c = (DOS_UMMA_ABL & 8) ? 0.f : num * rden[r];
                         pc[e] = c;
                         ox[e] = 2.f * c - ix[e]; oyr[e] = 2.f * c - yin; ozr[e] = 2.f * c - zin;
-                        any |= act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
+                        if (fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f) negm |= 1u << e;
                     }
-                    while (__any_sync(0xffffffffu, any)) {
-                        any = false;
+                    if (!act) negm = 0;
+                    if constexpr (C0 == 0) TRACE(4);
+                    // Set-to-zero fixup with rebalance, angle by angle but only for angles some lane of the warp needs it
+                    // for: all lanes run the pass in lock-step (a lane with nothing new to pin reproduces its values).
+                    if (__any_sync(0xffffffffu, negm != 0)) {
 #pragma unroll
                         for (int e = 0; e < N; ++e) {
-                            const float4 cc = cdd4[C0 + e];
-                            const float gx = ox[e] > 0.f ? 1.f : 0.f, gy = oyr[e] > 0.f ? 1.f : 0.f, gz = ozr[e] > 0.f ? 1.f : 0.f;
-                            const float hx = cc.x * ix[e], hy = cc.y * yi[e], hz = cc.z * zi[e];
-                            const float num = fmaf(fmaf(0.5f, gx, 0.5f), hx, fmaf(fmaf(0.5f, gy, 0.5f), hy, fmaf(fmaf(0.5f, gz, 0.5f), hz, qd[e])));
-                            const float den = fmaf(gx, cc.x, fmaf(gy, cc.y, fmaf(gz, cc.z, sig0)));
-                            const float c = __fdividef(num, den);
-                            pc[e] = c;
-                            ox[e] = gx * (2.f * c - ix[e]);
-                            oyr[e] = gy * (2.f * c - yi[e]);
-                            ozr[e] = gz * (2.f * c - zi[e]);
-                            any |= act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
+                            bool neg = (negm >> e) & 1u;
+                            while (__any_sync(0xffffffffu, neg)) {
+                                const float4 cc = cdd4[C0 + e];
+                                const float gx = ox[e] > 0.f ? 1.f : 0.f, gy = oyr[e] > 0.f ? 1.f : 0.f, gz = ozr[e] > 0.f ? 1.f : 0.f;
+                                const float hx = cc.x * ix[e], hy = cc.y * yi[e], hz = cc.z * zi[e];
+                                const float num = fmaf(fmaf(0.5f, gx, 0.5f), hx, fmaf(fmaf(0.5f, gy, 0.5f), hy, fmaf(fmaf(0.5f, gz, 0.5f), hz, qd[e])));
+                                const float den = fmaf(gx, cc.x, fmaf(gy, cc.y, fmaf(gz, cc.z, sig0)));
+                                const float c = __fdividef(num, den);
+                                pc[e] = c;
+                                ox[e] = gx * (2.f * c - ix[e]);
+                                oyr[e] = gy * (2.f * c - yi[e]);
+                                ozr[e] = gz * (2.f * c - zi[e]);
+                                neg = act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
+                            }
                         }
                     }
+                    if constexpr (C0 == 0) TRACE(5);
+                    // Lanes outside their x range compute on whatever they hold: nothing reads it (their neighbours are
+                    // outside too, their rows are skipped by the read-back, their stores are predicated off, and px is
+                    // re-seeded from the boundary value at the lane's first cell).
                     float hi[N], lo[N];
 #pragma unroll
                     for (int e = 0; e < N; ++e) {
                         const int r = C0 + e;
-                        if (act) {
-                            px[r] = ox[e]; oy[r] = oyr[e]; oz[r] = ozr[e];
-                            if (store_y) __stcg(fy_st + r * DOS_TK, oyr[e]);
-                            if (store_z) __stcg(fz_st + r * DOS_TJ, ozr[e]);
-                            if (last_x) __stcg(p.bx_out + ((size_t)o * A + a0 + r) * bxs + bxi, ox[e]);
-                        }
-                        tf32_split(act ? pc[e] : 0.f, hi[e], lo[e]);
+                        px[r] = ox[e]; oy[r] = oyr[e]; oz[r] = ozr[e];
+                        if (st_y) __stcg(fy_st + r * DOS_TK, oyr[e]);
+                        if (st_z) __stcg(fz_st + r * DOS_TJ, ozr[e]);
+                        if constexpr (REFL)
+                            if (last_x) __stcg(mv(p.bx_out) + ((size_t)o * A + a0 + r) * bxs + bxi, ox[e]);
+                        tf32_split(pc[e], hi[e], lo[e]);
                     }
                     if constexpr (C0 == 0) {
-                        TRACE(3);
                         wait_bar(&psi_empty[gs % PSL], ((gs / PSL) & 1) ^ 1, &s_abort, p.abort_flag, 32);
                         tc_fence_after();
-                        TRACE(4);
                     }
                     tmem_st_n<N>(tp + C0, hi);
                     tmem_st_n<N>(tp + A8 + C0, lo);
+                    if constexpr (C0 == 0) TRACE(6);
                 };
                 [&]<int... I>(std::integer_sequence<int, I...>) { (chunk.template operator()<I * CH>(), ...); }(
                     std::make_integer_sequence<int, (AG + CH - 1) / CH>{});
@@ -614,9 +638,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                     mbar_arrive(&psi_full[gs % PSL]);
                     st_release_cta(&s_prog[warp], t + 1);
                 }
-                TRACE(5);
                 if (t + SA < T) split(t + SA);
-                TRACE(6);
                 if (t >= EB) readback(t - EB);
                 TRACE(7);
             }
@@ -637,7 +659,8 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
 // ------------------------------------------------------------------------------------------------
 typedef void (*sweep_u_fn)(const SweepUArgs);
 
-struct UShape { int ag, ng; sweep_u_fn fn; };
+struct UShape { int ag, ng; sweep_u_fn fn[2]; };      // [vacuum only, reflective faces]
+#define USHAPE(AG, NG) {AG, NG, {sweep_umma_kernel<AG, NG, false>, sweep_umma_kernel<AG, NG, true>}}
 
 static const UShape *umma_shape(int per_oct)
 {
@@ -647,9 +670,7 @@ static const UShape *umma_shape(int per_oct)
     // pays a fixed per-step cost (waits, arrivals, fences, its share of staging / split / read-back), so few warps with
     // many angles win until the chains get too long.
     static const UShape shapes[] = {
-        {1, 1, sweep_umma_kernel<1, 1>}, {1, 3, sweep_umma_kernel<1, 3>}, {2, 3, sweep_umma_kernel<2, 3>},
-        {2, 5, sweep_umma_kernel<2, 5>}, {3, 5, sweep_umma_kernel<3, 5>}, {3, 7, sweep_umma_kernel<3, 7>},
-        {4, 7, sweep_umma_kernel<4, 7>}, {12, 3, sweep_umma_kernel<12, 3>},
+        USHAPE(1, 1), USHAPE(1, 3), USHAPE(2, 3), USHAPE(2, 5), USHAPE(3, 5), USHAPE(7, 3), USHAPE(7, 4), USHAPE(12, 3),
     };
     for (const UShape &s : shapes)
         if (s.ag * s.ng == per_oct) return &s;
@@ -668,7 +689,8 @@ static size_t umma_smem(int MP, int A, int n_mat)
     auto up = [](size_t b) { return (b + 127) & ~(size_t)127; };
     return up((size_t)RAW * 128 * MP * 4) + up((size_t)ASL * 2 * 16 * NCH * 128) + up((size_t)2 * (NAP / 8) * NCH * 128) +
            up((size_t)2 * (NMP / 8) * (A8 / 4) * 128) + up((size_t)RFU * 4 * A * DOS_TK * 4) + up((size_t)RFU * 4 * A * DOS_TJ * 4) +
-           up((size_t)A * 16) + up((size_t)n_mat * A * 4) + up((size_t)n_mat * 4) + up((size_t)8 * MP * 4) + up(64 * 8) + up(32 * 4) + 128;
+           up((size_t)A * 16) + up((size_t)n_mat * A * 4) + up((size_t)n_mat * 4) + up((size_t)8 * MP * 4) + up((size_t)A * DOS_TJ * 4) +
+           up(64 * 8) + up(32 * 4) + 128;
 }
 
 cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int *grid_out)
@@ -676,8 +698,9 @@ cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int 
     const UShape *s = umma_shape(per_oct);
     if (!s) return cudaErrorInvalidValue;
     const size_t smem = umma_smem(dos_mpad(L), per_oct, n_mat);
-    cudaError_t e = cudaFuncSetAttribute(s->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    cudaError_t e = cudaSuccess;
+    for (int v = 0; v < 2; ++v)
+        if ((e = cudaFuncSetAttribute(s->fn[v], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
@@ -691,6 +714,6 @@ cudaError_t dos_launch_sweep_umma(const SweepUArgs &a, int L, int grid, cudaStre
     const UShape *s = umma_shape(a.per_oct);
     if (!s) return cudaErrorInvalidValue;
     const size_t smem = umma_smem(dos_mpad(L), a.per_oct, a.n_mat);
-    s->fn<<<grid, (4 * s->ng + 4) * 32, smem, st>>>(a);
+    s->fn[a.refl ? 1 : 0]<<<grid, (4 * s->ng + 4) * 32, smem, st>>>(a);
     return cudaGetLastError();
 }
