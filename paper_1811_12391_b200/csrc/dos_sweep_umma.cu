@@ -90,9 +90,8 @@ __device__ __forceinline__ void red_add_v4(float *p, float a, float b, float c, 
 // instructions than the sixteen compute warps doing the work. So: one poll, then sleep between polls.
 // A hand-off that never arrives must not hang the GPU: the waiter sets the CTA's and the launch's abort flags and
 // everything drains with invalid results (dos_check then reports DOS_ERR_CUDA).
-__device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_abort, int *g_abort, unsigned sleep_ns = 64)
+__device__ __forceinline__ void wait_more(uint64_t *bar, unsigned parity, int *s_abort, int *g_abort, unsigned sleep_ns)
 {
-    if (mbar_try_wait(bar, parity)) return;
 #pragma unroll 1
     for (int outer = 0; outer < WAIT_LIMIT / 1024; ++outer) {
 #pragma unroll 1
@@ -105,6 +104,11 @@ __device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_
     *(volatile int *)s_abort = 1;
     atomicExch(g_abort, 1);
 }
+__device__ __forceinline__ void wait_bar(uint64_t *bar, unsigned parity, int *s_abort, int *g_abort, unsigned sleep_ns = 64)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    wait_more(bar, parity, s_abort, g_abort, sleep_ns);
+}
 
 // hi = x rounded to TF32 (round half away from zero on the bit pattern; inputs are finite), lo = x - hi (exact in
 // fp32; the tensor core reads its leading 11 bits: an error <= 2^-22 |x|)
@@ -113,6 +117,18 @@ __device__ __forceinline__ void tf32_split(float x, float &hi, float &lo)
     hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
     lo = x - hi;
 }
+
+// Register re-allocation (setmaxnreg; warp roles come in aligned groups of 4 warps, as it requires). The launch gives
+// every thread R0 = 64K / threads registers (multiple of 8); the 4 helper warps keep 40 and the 4 NG compute warps share
+// what that frees. setmaxnreg re-divides the CTA's OWN allocation: asking for more than the launch total blocks for
+// ever, so dos_sweep_umma_grid checks the launch's register count against these numbers before anything runs.
+__host__ __device__ constexpr int umma_reg_launch(int ng) { return (65536 / ((4 * ng + 4) * 32)) / 8 * 8 > 255 ? 248 : (65536 / ((4 * ng + 4) * 32)) / 8 * 8; }
+__host__ __device__ constexpr int umma_reg_helper() { return 40; }
+__host__ __device__ constexpr int umma_reg_compute(int ng) { return umma_reg_launch(ng) + (umma_reg_launch(ng) - umma_reg_helper()) / ng / 8 * 8; }
+#ifndef DOS_UMMA_REALLOC
+#define DOS_UMMA_REALLOC 1
+#endif
+__host__ __device__ constexpr bool umma_realloc(int ag, int ng) { return DOS_UMMA_REALLOC && ng >= 2 && ag >= 7; }
 
 struct Geom {          // one octant's (j,k) column of this lane
     bool valid;
@@ -160,7 +176,8 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
     size_t sh = 0;           // byte offset of the item's problem of the position batch: Q, phi, faces, boundaries, done
     auto mv = [&sh](auto *ptr) { return reinterpret_cast<decltype(ptr)>(reinterpret_cast<size_t>(ptr) + sh); };
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int A = p.per_oct, MP = p.MP, KP = (MP + 7) & ~7, NCH = KP / 4, A8 = (A + 7) & ~7, NAP = (A + 15) & ~15, NMP = (MP + 15) & ~15;
+    constexpr int A = AG * NG, A8 = (A + 7) & ~7, NAP = (A + 15) & ~15;      // the host picks the instance with AG * NG = per_oct
+    const int MP = p.MP, KP = (MP + 7) & ~7, NCH = KP / 4, NMP = (MP + 15) & ~15;
     constexpr int NCW = 4 * NG;
     // ---- shared memory carve-up (every piece a multiple of 128 bytes) ----
     unsigned char *sp = smem_raw;
@@ -180,11 +197,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
     int *s_prog = reinterpret_cast<int *>(carve(32 * 4));                                       // [NCW] steps finished per compute warp
     uint64_t *raw_full = bars;            // [RAW][4 octants]
     uint64_t *a_full = bars + 16;         // [ASL]
-    uint64_t *a_empty = bars + 18;
     uint64_t *q_full = bars + 20;         // [DQS]
     uint64_t *q_empty = bars + 24;
     uint64_t *psi_full = bars + 28;       // [PSL]
-    uint64_t *psi_empty = bars + 30;
     uint64_t *phi_full = bars + 32;       // [DPS]
     uint64_t *phi_empty = bars + 34;
     uint64_t *fin_full = bars + 36;       // [RFU]
@@ -207,9 +222,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
     for (int i = tid; i < A * DOS_TJ; i += blockDim.x) s_zero[i] = 0.f;
     if (tid == 0) {
         for (int i = 0; i < 16; ++i) mbar_init(&raw_full[i], 32 * NG);      // one cp.async arrival per thread of the octant's warps
-        for (int i = 0; i < ASL; ++i) { mbar_init(&a_full[i], NCW); mbar_init(&a_empty[i], 1); }
+        for (int i = 0; i < ASL; ++i) mbar_init(&a_full[i], NCW);
         for (int i = 0; i < DQS; ++i) { mbar_init(&q_full[i], 1); mbar_init(&q_empty[i], NCW); }
-        for (int i = 0; i < PSL; ++i) { mbar_init(&psi_full[i], NCW); mbar_init(&psi_empty[i], 1); }
+        for (int i = 0; i < PSL; ++i) mbar_init(&psi_full[i], NCW);
         for (int i = 0; i < DPS; ++i) { mbar_init(&phi_full[i], 1); mbar_init(&phi_empty[i], NCW); }
         for (int i = 0; i < RFU; ++i) mbar_init(&fin_full[i], 1);
         s_abort = 0;
@@ -261,7 +276,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
         return true;
     };
 
+    constexpr bool REALLOC = umma_realloc(AG, NG);
     if (is_service) {
+        if constexpr (REALLOC) setmaxnreg_dec<umma_reg_helper()>();
         while (next_item()) {
             // ------- service warp: publishes this item's progress, follows the two upwind items' progress -------
             const bool up_tile_y = tj > 0, up_tile_z = tk > 0;       // boundary inflow (reflective) needs no hand-off
@@ -306,6 +323,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             gs0 += T;
         }
     } else if (is_feed) {
+        if constexpr (REALLOC) setmaxnreg_dec<umma_reg_helper()>();
         while (next_item()) {
             // ------- feeder warp: bulk copies of the tile-inflow faces the upwind tiles have published -------
             // step s of octant qq needs fy_in[s][A][TK] and fz_in[s][A][TJ]: two contiguous blocks per octant.
@@ -350,6 +368,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             gs0 += T;
         }
     } else if (is_m2d) {
+        if constexpr (REALLOC) setmaxnreg_dec<umma_reg_helper()>();
         while (next_item()) {
             // ------- M2D issuer: D_q[slot] = A_lo B_hi + A_hi B_lo + A_hi B_hi -------
             __syncthreads();                          // S2
@@ -371,12 +390,24 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                     const unsigned a0 = smem_u32(s_a) + (gs % ASL) * a_slot_bytes;
                     const uint64_t adh = umma_smem_desc(a0, 128, NCH * 128), adl = umma_smem_desc(a0 + a_half, 128, NCH * 128);
                     const unsigned d = tm_dq + (gs % DQS) * NAP;
-                    const int nk = KP / 8;
-                    for (int ks = 0; ks < nk; ++ks) umma_ss_if(on, d, adl + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, ks ? 1u : 0u);
-                    for (int ks = 0; ks < nk; ++ks) umma_ss_if(on, d, adh + (uint64_t)(ks * 16), bdl + (uint64_t)(ks * 16), idesc, 1u);
-                    for (int ks = 0; ks < nk; ++ks) umma_ss_if(on, d, adh + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, 1u);
+                    // K / 8 instructions per term, unrolled for the K of P0, P2-P3, P4-P5 (the issue is a serial chain
+                    // in one thread: every instruction saved shortens the path split -> M2D -> cell update)
+                    auto issue = [&]<int NK>() {
+#pragma unroll
+                        for (int ks = 0; ks < NK; ++ks) umma_ss_if(on, d, adl + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, ks ? 1u : 0u);
+#pragma unroll
+                        for (int ks = 0; ks < NK; ++ks) umma_ss_if(on, d, adh + (uint64_t)(ks * 16), bdl + (uint64_t)(ks * 16), idesc, 1u);
+#pragma unroll
+                        for (int ks = 0; ks < NK; ++ks) umma_ss_if(on, d, adh + (uint64_t)(ks * 16), bdh + (uint64_t)(ks * 16), idesc, 1u);
+                    };
+                    switch (KP / 8) {
+                    case 1: issue.template operator()<1>(); break;
+                    case 2: issue.template operator()<2>(); break;
+                    case 4: issue.template operator()<4>(); break;
+                    default: issue.template operator()<5>(); break;
+                    }
+                    // the accumulator is ready, and with it the A slot is free again (one commit tells both)
                     umma_commit_if(leader ? 1u : 0u, &q_full[gs % DQS]);
-                    umma_commit_if(leader ? 1u : 0u, &a_empty[gs % ASL]);
                 }
                 __syncwarp();
                 TRACE(3);
@@ -384,6 +415,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             gs0 += T;
         }
     } else if (is_d2m) {
+        if constexpr (REALLOC) setmaxnreg_dec<umma_reg_helper()>();
         while (next_item()) {
             // ------- D2M issuer: D_phi[slot] = psi_lo B_hi + psi_hi B_lo + psi_hi B_hi (A operand in TMEM) -------
             __syncthreads();                          // S2
@@ -404,12 +436,15 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                     const unsigned on = (leader && !(DOS_UMMA_ABL & 4)) ? 1u : 0u;
                     const unsigned ah = tm_psi + (gs % PSL) * 2 * A8, al = ah + A8;
                     const unsigned d = tm_dphi + (gs % DPS) * NMP;
-                    const int nk = A8 / 8;
+                    constexpr int nk = A8 / 8;
+#pragma unroll
                     for (int ks = 0; ks < nk; ++ks) umma_ts_if(on, d, al + ks * 8, bdh + (uint64_t)(ks * 16), idesc, ks ? 1u : 0u);
+#pragma unroll
                     for (int ks = 0; ks < nk; ++ks) umma_ts_if(on, d, ah + ks * 8, bdl + (uint64_t)(ks * 16), idesc, 1u);
+#pragma unroll
                     for (int ks = 0; ks < nk; ++ks) umma_ts_if(on, d, ah + ks * 8, bdh + (uint64_t)(ks * 16), idesc, 1u);
+                    // D_phi is ready, and with it the psi operand slot is free again
                     umma_commit_if(leader ? 1u : 0u, &phi_full[gs % DPS]);
-                    umma_commit_if(leader ? 1u : 0u, &psi_empty[gs % PSL]);
                 }
                 __syncwarp();
                 TRACE(3);
@@ -418,6 +453,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
         }
     } else {
         // ---------------- compute warps ----------------
+        if constexpr (REALLOC) setmaxnreg_inc<umma_reg_compute(NG)>();
         while (next_item()) {
             const int o = quad * 4 + q;               // this warp's octant; the lane owns one (j,k) column of its tile
             const Geom g = make_geom(p, o, tj, tk, lane);
@@ -438,33 +474,52 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                            ((long long)(-kst) * A + a0) * DOS_TJ;
             const int fy_inc = A * DOS_TK, fz_inc = A * DOS_TJ;
             const float *finy0 = s_finy + (q * A + a0) * DOS_TK + kk, *finz0 = s_finz + (q * A + a0) * DOS_TJ + jj;
-            const uint8_t *mat_p = p.mat + g.cbase;
             const int istep = g.istep, t_lo = g.t_lo;
-            const long long cinc = (long long)istep * MP;                // floats between this lane's consecutive cells
-            const float *qsrc = mv(p.Q) + g.cbase * MP;
-            float *phi_base = mv(p.phi) + g.cbase * MP;
             const unsigned *sgn = s_sign + o * MP;
-            const int nq = MP / 4;                                       // 16-byte pieces of a row; this warp takes grp, grp + NG, ...
+            const int nq = MP / 4;                                       // 16-byte pieces of a row
+            // Global traffic is laid out piece-major, not row-major: the octant's 32 rows of a step are 32 nq pieces of
+            // 16 bytes; lane l of the octant's warp grp moves pieces (k NG + grp) 32 + l. Consecutive lanes then touch
+            // consecutive 16 bytes of the same row (2-3 lines per row) where "lane = row" costs one L1 wavefront per
+            // lane and piece: measured, those wavefronts (~2 cycles each, ~3000 per step) were the sweep's bound.
+            // Per piece: its 16-byte offset in Q / phi at step 0 and (piece index in the row) << 16 | (row's first step).
+            constexpr int KPL = (9 + NG - 1) / NG;
+            int poff[KPL];
+            unsigned pmeta[KPL];
+#pragma unroll
+            for (int k = 0; k < KPL; ++k) {
+                const int i = (k * NG + grp) * 32 + lane, r = i / nq, c = i - r * nq;
+                const Geom gr = make_geom(p, o, tj, tk, r & 31);
+                const bool ok = i < 32 * nq && gr.valid;
+                poff[k] = ok ? (int)((gr.cbase * MP + 4 * c) >> 2) : 0;
+                pmeta[k] = ok ? ((unsigned)c << 16) | (unsigned)gr.t_lo : 0x7fffu;
+            }
+            const int cstep16 = istep * nq;                              // 16-byte units between a column's consecutive cells
+            const float *Qb = mv(p.Q);
+            float *phib = mv(p.phi);
+            // material ids: the column's cells are consecutive bytes, so one aligned 32-bit load serves 4 steps
+            const int jp_ = tj * DOS_TJ + jj, kp_ = tk * DOS_TK + kk;
+            const int jg = (o & 2) ? p.ny - 1 - jp_ : jp_, kg = (o & 4) ? p.nz - 1 - kp_ : kp_;
+            const uint8_t *mat_col = p.mat + (g.valid ? ((size_t)kg * p.ny + jg) * nx : 0);
+            const bool mat4 = (nx & 3) == 0;
             __syncthreads();                          // S2
             const float4 *cdd4 = reinterpret_cast<const float4 *>(s_cdd) + a0;     // (cx, cy, cz, cx+cy+cz) per angle: warp-uniform reads
 
             // staging: this lane's pieces of its row of step s, by cp.async; the thread's arrival on the ring slot's
             // mbarrier fires when they have landed
             auto stage = [&](int s) {
-                const bool on = (unsigned)(s - t_lo) < (unsigned)nx;
                 const unsigned gsx = gs0 + s;
-                if (on && !(DOS_UMMA_ABL & 1)) {
-                    float *dst = s_raw + ((size_t)(gsx % RAW) * 128 + row) * MP;
-                    const float *src = qsrc + cinc * s;
-                    for (int c = grp; c < nq; c += NG) cp_async16(dst + 4 * c, src + 4 * c);
-                }
+                float *dst = s_raw + ((size_t)(gsx % RAW) * 128 + q * 32) * MP + 4 * (grp * 32 + lane);
+#pragma unroll
+                for (int k = 0; k < KPL; ++k)
+                    if ((unsigned)(s - (int)(pmeta[k] & 0xffffu)) < (unsigned)nx && !(DOS_UMMA_ABL & 1))
+                        cp_async16(dst + k * (NG * 128), Qb + ((long long)poff[k] + (long long)cstep16 * s) * 4);
                 cp_async_mbar_arrive(&raw_full[(gsx % RAW) * 4 + q]);
             };
             // split: this lane's pieces of its row of step s -> mirror signs, TF32 hi / lo, UMMA layout -> a_full
-            auto split = [&](int s) {
+            // (the A slot of step s was last read by the M2D of step s - ASL: the caller has seen that one's q_full)
+            auto split = [&](int s, bool landed) {
                 const unsigned gsx = gs0 + s;
-                wait_bar(&raw_full[(gsx % RAW) * 4 + q], (gsx / RAW) & 1, &s_abort, p.abort_flag, 32);
-                wait_bar(&a_empty[gsx % ASL], ((gsx / ASL) & 1) ^ 1, &s_abort, p.abort_flag, 32);
+                if (!landed) wait_more(&raw_full[(gsx % RAW) * 4 + q], (gsx / RAW) & 1, &s_abort, p.abort_flag, 32);
                 const bool on = (unsigned)(s - t_lo) < (unsigned)nx;
                 const float4 *src = reinterpret_cast<const float4 *>(s_raw + ((size_t)(gsx % RAW) * 128 + row) * MP);
                 // element (row, piece c): ((row / 8) * NCH + c) * 32 + (row % 8) * 4 floats
@@ -475,59 +530,95 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&a_full[gsx % ASL]);
             };
-            // read-back: this warp's 4-column groups of D_phi of step s -> mirror signs -> red.global.add.v4 into phi
-            auto readback = [&](int s) {
+            // read-back: D_phi of step s leaves tensor memory row by row (lane = row: this warp's pieces grp, grp + NG, ..),
+            // is turned piece-major through shared memory, gets the mirror signs and goes into phi with red.global.add.v4.
+            // The turning buffer is the staging slot the split of step s + EB + SA has just consumed: this warp writes
+            // only the pieces it read there itself; the octant's warps meet in a named barrier before they read each
+            // other's pieces, and that same barrier one step later orders these reads before the slot's next cp.async.
+            auto readback = [&](int s, bool ready) {
                 const unsigned gsx = gs0 + s;
-                wait_bar(&phi_full[gsx % DPS], (gsx / DPS) & 1, &s_abort, p.abort_flag, 32);
+                if (!ready) wait_more(&phi_full[gsx % DPS], (gsx / DPS) & 1, &s_abort, p.abort_flag, 32);
                 tc_fence_after();
-                const bool on = (unsigned)(s - t_lo) < (unsigned)nx;
                 const unsigned ta = tm_dphi + lane_base + (gsx % DPS) * NMP;
-                float *phi_p = phi_base + cinc * s;
-                for (int c = grp; c < nq; c += NG) {
-                    float v[4];
-                    tmem_ld<4>(ta + 4 * c, v);
+                float *rb = s_raw + ((size_t)((gsx + EB + SA) % RAW) * 128 + q * 32) * MP;
+                float4 *mine = reinterpret_cast<float4 *>(rb + lane * MP);
+                for (int c = grp; c < nq; c += 3 * NG) {      // three pieces in flight per tcgen05.wait::ld (warp-uniform conditions)
+                    float v0[4], v1[4], v2[4];
+                    tmem_ld<4>(ta + 4 * c, v0);
+                    if (c + NG < nq) tmem_ld<4>(ta + 4 * (c + NG), v1);
+                    if (c + 2 * NG < nq) tmem_ld<4>(ta + 4 * (c + 2 * NG), v2);
                     tmem_wait_ld();
-                    if (on && !(DOS_UMMA_ABL & 2)) {
-                        const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn + 4 * c);
-                        red_add_v4(phi_p + 4 * c, __uint_as_float(__float_as_uint(v[0]) ^ s4.x), __uint_as_float(__float_as_uint(v[1]) ^ s4.y),
-                                   __uint_as_float(__float_as_uint(v[2]) ^ s4.z), __uint_as_float(__float_as_uint(v[3]) ^ s4.w));
-                    }
+                    mine[c] = make_float4(v0[0], v0[1], v0[2], v0[3]);
+                    if (c + NG < nq) mine[c + NG] = make_float4(v1[0], v1[1], v1[2], v1[3]);
+                    if (c + 2 * NG < nq) mine[c + 2 * NG] = make_float4(v2[0], v2[1], v2[2], v2[3]);
                 }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&phi_empty[gsx % DPS]);
+                if constexpr (NG > 1) asm volatile("bar.sync %0, %1;" ::"r"(1 + q), "n"(32 * NG) : "memory");
+                const float4 *pm = reinterpret_cast<const float4 *>(rb) + grp * 32 + lane;
+#pragma unroll
+                for (int k = 0; k < KPL; ++k)
+                    if ((unsigned)(s - (int)(pmeta[k] & 0xffffu)) < (unsigned)nx && !(DOS_UMMA_ABL & 2)) {
+                        const float4 v = pm[k * (NG * 32)];
+                        const uint4 s4 = *reinterpret_cast<const uint4 *>(sgn + 4 * (pmeta[k] >> 16));
+                        red_add_v4(phib + ((long long)poff[k] + (long long)cstep16 * s) * 4, __uint_as_float(__float_as_uint(v.x) ^ s4.x),
+                                   __uint_as_float(__float_as_uint(v.y) ^ s4.y), __uint_as_float(__float_as_uint(v.z) ^ s4.z),
+                                   __uint_as_float(__float_as_uint(v.w) ^ s4.w));
+                    }
             };
 
             // x faces: the column's inflow is vacuum or the mirror octant's outflow of the previous sweep
             // (reflective); px starts as that inflow and is only touched while the lane is active
-            const int jp_ = tj * DOS_TJ + jj, kp_ = tk * DOS_TK + kk;
-            const int jg = (o & 2) ? p.ny - 1 - jp_ : jp_, kg = (o & 4) ? p.nz - 1 - kp_ : kp_;
             const size_t bxi = g.valid ? (size_t)kg * p.ny + jg : 0, bxs = (size_t)p.nz * p.ny;
             const bool refl_x = (refl & 1) && g.valid;
             const int t_last = g.valid ? t_lo + nx - 1 : -1;
             float px[AG], oy[AG], oz[AG];
 #pragma unroll
             for (int r = 0; r < AG; ++r) px[r] = oy[r] = oz[r] = 0.f;
-            auto mat_of = [&](int s) -> int { return ((unsigned)(s - t_lo) < (unsigned)nx) ? min((int)__ldg(mat_p + (long long)istep * s), p.n_mat - 1) : 0; };
-            int m_cur = mat_of(0), m_nxt = mat_of(1);
+            // material word of the next 4 cells in travel order, fetched 3 steps before its first cell (nx % 4 != 0: bytes)
+            auto mat_word = [&](int xl) -> unsigned {       // xl: first cell of the word, counted along the travel direction
+                return __ldg(reinterpret_cast<const unsigned *>(mat_col + (istep > 0 ? xl : nx - 4 - xl)));
+            };
+            unsigned mw = 0, mw_nxt = (mat4 && g.valid) ? mat_word(0) : 0;
             for (int s = 0; s < LA && s < T; ++s) stage(s);
-            for (int s = 0; s < SA && s < T; ++s) split(s);
+            for (int s = 0; s < SA && s < T; ++s) split(s, false);
 
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
                 const bool act = (unsigned)(t - t_lo) < (unsigned)nx;
-                const int m0 = m_cur;
-                m_cur = m_nxt;
-                m_nxt = mat_of(t + 2);
+                const int xl = t - t_lo;              // the lane's cell of this step, counted along the travel direction
+                int m0 = 0;
+                if (mat4) {
+                    if (act && (xl & 3) == 0) mw = mw_nxt;
+                    if (act && (xl & 3) == 1 && xl + 3 < nx) mw_nxt = mat_word(xl + 3);
+                    m0 = (int)((mw >> (8 * (istep > 0 ? (xl & 3) : 3 - (xl & 3)))) & 255u);
+                } else if (act) {
+                    m0 = (int)__ldg(mat_col + (istep > 0 ? xl : nx - 1 - xl));
+                }
+                m0 = min(m0, p.n_mat - 1);
                 TRACE(0);
+                // The step's four hand-offs are polled up front, together (a try_wait takes ~100 cycles to answer even
+                // when the phase is long over); whatever has not arrived yet is waited for where it is needed.
+                const unsigned fs = fs0 + t;
+                const bool have_in = has_y || has_z, do_split = t + SA < T, do_rb = t >= EB;
+                const bool r_q = mbar_try_wait(&q_full[gs % DQS], (gs / DQS) & 1);
+                const bool r_f = have_in ? mbar_try_wait(&fin_full[fs % RFU], (fs / RFU) & 1) : true;
+                const bool r_r = do_split ? mbar_try_wait(&raw_full[((gs + SA) % RAW) * 4 + q], ((gs + SA) / RAW) & 1) : true;
+                const bool r_p = do_rb ? mbar_try_wait(&phi_full[(gs - EB) % DPS], ((gs - EB) / DPS) & 1) : true;
                 if (t + LA < T) stage(t + LA);
-                wait_bar(&q_full[gs % DQS], (gs / DQS) & 1, &s_abort, p.abort_flag, 32);
+                if (!r_q) wait_more(&q_full[gs % DQS], (gs / DQS) & 1, &s_abort, p.abort_flag, 32);
                 TRACE(1);
                 tc_fence_after();
-                const unsigned fs = fs0 + t;
-                if (has_y || has_z) wait_bar(&fin_full[fs % RFU], (fs / RFU) & 1, &s_abort, p.abort_flag, 32);
+                // M2D of step t is done: its A slot takes the split of step t + SA (so that M2D has a whole cell update
+                // of lead); D2M of step t - EB is done once its D_phi is there: its psi slot is the one this step writes
+                if (do_split) split(t + SA, r_r);
                 TRACE(2);
+                if (do_rb) readback(t - EB, r_p);
+                TRACE(3);
+                if (!r_f) wait_more(&fin_full[fs % RFU], (fs / RFU) & 1, &s_abort, p.abort_flag, 32);
+                TRACE(4);
                 const int fslot = (int)(fs % RFU) * 4 * A;
                 const float *rden = s_rden + m0 * A + a0;
                 const float sig0 = s_sig[m0];
@@ -553,15 +644,29 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 // Each chunk reads its columns of the discrete source from tensor memory and writes its psi_c (TF32
                 // hi + lo) back as the D2M's A operand, so no per-angle array outlives a chunk except the 3 face fluxes.
 #ifndef DOS_UMMA_CH
-#define DOS_UMMA_CH 4
+#define DOS_UMMA_CH 3
 #endif
-                constexpr int CH = AG <= DOS_UMMA_CH ? AG : (AG % DOS_UMMA_CH == 0 ? DOS_UMMA_CH : (AG % 3 == 0 ? 3 : 4));
+                // (the reflective variant of the widest shape is short of registers: smaller chunks, no prefetch)
+                constexpr bool TIGHT = REFL && AG >= 12;
+                constexpr int CHW = TIGHT ? 3 : DOS_UMMA_CH;
+                constexpr int CH = AG <= CHW ? AG : (AG % CHW == 0 ? CHW : (AG % 3 == 0 ? 3 : 4));
+#ifndef DOS_UMMA_QPF
+#define DOS_UMMA_QPF 0
+#endif
+                float qn[CH];                         // the next chunk's columns of D_q, in flight while this chunk computes
+                if constexpr (DOS_UMMA_QPF && !TIGHT) tmem_ld_n<(AG < CH ? AG : CH)>(tq, qn);
                 auto chunk = [&]<int C0>() {
                     constexpr int N = AG - C0 < CH ? AG - C0 : CH;
                     float qd[N], ix[N], yi[N], zi[N], ox[N], oyr[N], ozr[N], pc[N];
-                    tmem_ld_n<N>(tq + C0, qd);
-                    tmem_wait_ld();
-                    if constexpr (C0 == 0) TRACE(3);
+                    if constexpr (DOS_UMMA_QPF && !TIGHT) {
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < N; ++e) qd[e] = qn[e];
+                        if constexpr (C0 + CH < AG) tmem_ld_n<(AG - C0 - CH < CH ? AG - C0 - CH : CH)>(tq + C0 + CH, qn);
+                    } else {
+                        tmem_ld_n<N>(tq + C0, qd);
+                        tmem_wait_ld();
+                    }
                     unsigned negm = 0;                // bit e: angle e of the chunk has a negative outflow in this (active) lane
 #pragma unroll
                     for (int e = 0; e < N; ++e) {
@@ -582,7 +687,6 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                         if (fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f) negm |= 1u << e;
                     }
                     if (!act) negm = 0;
-                    if constexpr (C0 == 0) TRACE(4);
                     // Set-to-zero fixup with rebalance, angle by angle but only for angles some lane of the warp needs it
                     // for: all lanes run the pass in lock-step (a lane with nothing new to pin reproduces its values).
                     if (__any_sync(0xffffffffu, negm != 0)) {
@@ -604,7 +708,6 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                             }
                         }
                     }
-                    if constexpr (C0 == 0) TRACE(5);
                     // Lanes outside their x range compute on whatever they hold: nothing reads it (their neighbours are
                     // outside too, their rows are skipped by the read-back, their stores are predicated off, and px is
                     // re-seeded from the boundary value at the lane's first cell).
@@ -619,17 +722,14 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                             if (last_x) __stcg(mv(p.bx_out) + ((size_t)o * A + a0 + r) * bxs + bxi, ox[e]);
                         tf32_split(pc[e], hi[e], lo[e]);
                     }
-                    if constexpr (C0 == 0) {
-                        wait_bar(&psi_empty[gs % PSL], ((gs / PSL) & 1) ^ 1, &s_abort, p.abort_flag, 32);
-                        tc_fence_after();
-                    }
                     tmem_st_n<N>(tp + C0, hi);
                     tmem_st_n<N>(tp + A8 + C0, lo);
-                    if constexpr (C0 == 0) TRACE(6);
+                    if constexpr (C0 == 0) TRACE(5);
                 };
                 [&]<int... I>(std::integer_sequence<int, I...>) { (chunk.template operator()<I * CH>(), ...); }(
                     std::make_integer_sequence<int, (AG + CH - 1) / CH>{});
                 fy_st += fy_inc; fz_st += fz_inc;
+                TRACE(6);
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();                         // also orders every lane's face stores before the progress word
@@ -638,11 +738,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                     mbar_arrive(&psi_full[gs % PSL]);
                     st_release_cta(&s_prog[warp], t + 1);
                 }
-                if (t + SA < T) split(t + SA);
-                if (t >= EB) readback(t - EB);
                 TRACE(7);
             }
-            for (int s = T - EB > 0 ? T - EB : 0; s < T; ++s) readback(s);
+            for (int s = T - EB > 0 ? T - EB : 0; s < T; ++s) readback(s, false);
             gs0 += T;
             if (has_y || has_z) fs0 += T;
         }
@@ -670,7 +768,7 @@ static const UShape *umma_shape(int per_oct)
     // pays a fixed per-step cost (waits, arrivals, fences, its share of staging / split / read-back), so few warps with
     // many angles win until the chains get too long.
     static const UShape shapes[] = {
-        USHAPE(1, 1), USHAPE(1, 3), USHAPE(2, 3), USHAPE(2, 5), USHAPE(3, 5), USHAPE(7, 3), USHAPE(7, 4), USHAPE(12, 3),
+        USHAPE(1, 1), USHAPE(1, 3), USHAPE(2, 3), USHAPE(5, 2), USHAPE(5, 3), USHAPE(7, 3), USHAPE(14, 2), USHAPE(12, 3),
     };
     for (const UShape &s : shapes)
         if (s.ag * s.ng == per_oct) return &s;
@@ -699,8 +797,14 @@ cudaError_t dos_sweep_umma_grid(int L, int per_oct, int n_mat, int n_items, int 
     if (!s) return cudaErrorInvalidValue;
     const size_t smem = umma_smem(dos_mpad(L), per_oct, n_mat);
     cudaError_t e = cudaSuccess;
-    for (int v = 0; v < 2; ++v)
+    for (int v = 0; v < 2; ++v) {
         if ((e = cudaFuncSetAttribute(s->fn[v], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        if (umma_realloc(s->ag, s->ng)) {     // the launch must own the registers the roles re-divide (see umma_reg_*)
+            cudaFuncAttributes fa;
+            if ((e = cudaFuncGetAttributes(&fa, s->fn[v])) != cudaSuccess) return e;
+            if (fa.numRegs * (4 * s->ng + 4) < umma_reg_compute(s->ng) * 4 * s->ng + umma_reg_helper() * 4) return cudaErrorLaunchOutOfResources;
+        }
+    }
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
