@@ -209,8 +209,9 @@ def run_ours(args):
     job_updates = updates_all if sharded else world * updates_all               # what all ranks together process per step
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
+        n_batch = 2 if summed else max(1, min(args.batch, len(mine)))     # summed-source mode needs the n_batch > 1 buffers
         ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"],
-                          device=dev, stream=stream, n_batch=len(mine) if summed else 1)
+                          device=dev, stream=stream, n_batch=n_batch)
         dose = ctx.new_field(groups=False)
         flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
     ctx.dos_set_option("profile", 1)
@@ -239,23 +240,16 @@ def run_ours(args):
             step_summed()
             ctx.dos_dose_host(dose_host, accumulate=False)
             return
-        for n, s in enumerate(mine):
-            ctx.dos_uncollided(p["sources"][s], p["spectrum"])
-            ctx.dos_solve(p["n_iter"])
-            if n + 1 < len(mine):
-                ctx.dos_dose(dose, accumulate=(n > 0))
-        # the last position's dose is added on the device and the sum is copied to the host
         if len(mine) > 1 or sharded:
-            if mine:
-                ctx.dos_dose(dose, accumulate=(len(mine) > 1))
-            else:
-                dose.zero_()
+            scan.run_scan(ctx, p, mine, dose)         # doses of the positions summed on the device, the sum copied to the host
             with torch.cuda.stream(stream):           # the context's stream, not torch's current one: the copy must
                 if sharded:                           # come after the last dos_dose
                     scan.all_reduce_dose(dose)
                 dose_pinned.copy_(dose.reshape(-1), non_blocking=True)
             stream.synchronize()
         else:
+            ctx.dos_uncollided(p["sources"][mine[0]], p["spectrum"])
+            ctx.dos_solve(p["n_iter"])
             ctx.dos_dose_host(dose_host, accumulate=False)
 
     def l2_flush():
@@ -324,9 +318,11 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = _peaks()
         sweep_ms = prof["sweep_ms"] / max(prof["sweep_launches"], 1)
-        sweep_bytes = (12 * M + 1) * nv      # compulsory: read Q_fix[M] + phi_old[M], write phi_new[M] (fp32), 1 B material id
+        # problems per sweep launch: a position batch sweeps up to n_batch positions in one launch
+        per_launch = 1.0 if summed else len(mine) / max(1, -(-len(mine) // n_batch))
+        sweep_bytes = (12 * M + 1) * nv * per_launch     # compulsory: read Q_fix[M] + phi_old[M], write phi_new[M] (fp32), 1 B material id
         achieved = sweep_bytes / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
-        flop = (4 * M + 12) * nv * n_ang
+        flop = (4 * M + 12) * nv * n_ang * per_launch
         rt_ms = prof["raytrace_ms"] / max(prof["raytrace_launches"], 1)
         traffic = None
         sweep_name = "sweep_umma_kernel" if M >= 25 else "sweep_kernel"     # tensor-memory sweep from P4 up, FFMA sweep below
@@ -348,6 +344,7 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOADS[args.config] + (" -- summed-source mode: the positions form ONE source, one solve"
                                                              if summed else ""), "positions_per_rank": len(mine),
+                       "position_batch": n_batch,
                        "parallelism": ("source positions sharded over ranks, one all-reduce of the dose map" if sharded else
                                        "replicas only") if world > 1 else "1 gpu",
                        "l2": "flushed between timed steps (256 MiB fill)", "arithmetic": "fp32 sweep/sources/dose, fp64 ray trace"},
@@ -365,7 +362,8 @@ def run_ours(args):
                                  "algorithmic_flop_per_launch": flop},
                          "launch_ms": sweep_ms,
                          "launches": int(prof["sweep_launches"]), "share_of_step": prof["sweep_ms"] / total_ms if total_ms else None,
-                         "updates_per_s_in_kernel": nv * n_ang / (sweep_ms * 1e-3) if sweep_ms > 0 else 0.0},
+                         "updates_per_s_in_kernel": nv * n_ang * per_launch / (sweep_ms * 1e-3) if sweep_ms > 0 else 0.0,
+                         "problems_per_launch": per_launch},
             "raytrace": {"launch_ms": rt_ms, "launches": int(prof["raytrace_launches"]),
                          "achieved_gbs": (nv * (1 + 4 * p["n_group"])) / (rt_ms * 1e-3) / 1e9 if rt_ms > 0 else 0.0,
                          "hbm_frac": (nv * (1 + 4 * p["n_group"])) / (rt_ms * 1e-3) / 1e9 / peak if rt_ms > 0 else 0.0,
@@ -390,6 +388,7 @@ def main():
     ap.add_argument("--config", default="config5", choices=sorted(WORKLOADS),
                     help="default: config5, the largest single-GPU workload (BASELINE.json's metric is not quoted on a config)")
     ap.add_argument("--positions", type=int, default=0, help="config4 / paper_*: source positions per step (default 36 / 16)")
+    ap.add_argument("--batch", type=int, default=4, help="source positions swept together (dos_uncollided_batch); 1 = one by one")
     ap.add_argument("--sn", type=int, default=0, help="quadrature order override (paper_*: S2..S8)")
     ap.add_argument("--pl", type=int, default=None, help="scattering order override (paper_*: P0..P1)")
     ap.add_argument("--scan", default="separate", choices=["separate", "summed"],
