@@ -35,6 +35,7 @@ struct dos_ctx {
     const uint8_t *d_mat;        // current material grid (caller's or the workspace copy)
     char *ws;
     Layout lay;
+    std::vector<float> h_cdd;    // [per_oct][4] diamond-difference coefficients (host copy: travels in the sweep's parameters)
     std::vector<int> band_lo;    // [G]: lowest g' with a non-zero sigma_s^{g'->g}
     int state;                   // 0 created, 1 uncollided done, 2 solved
     bool can_sum, summed;        // workspace holds the summed-source buffers; the current uncollided state is a sum
@@ -280,7 +281,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->contraction_pref = 0;
     c->ag_pref = c->aux_pref = 0;
     c->asplit = default_asplit(per, c->n_items);
-    c->chunk = 4;
+    c->chunk = 2;
     c->two_per_sm = 1;
     c->umma = false;
     c->grid = c->grid_u = 0;
@@ -389,6 +390,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     if (e == cudaSuccess) e = up(lay.m2d, m2d.data(), sizeof(float) * m2d.size());
     if (e == cudaSuccess) e = up(lay.d2m, d2m.data(), sizeof(float) * d2m.size());
     if (e == cudaSuccess) e = up(lay.cdd, cdd.data(), sizeof(float) * cdd.size());
+    c->h_cdd = cdd;
     if (e == cudaSuccess) e = up(lay.items, items.data(), sizeof(int) * items.size());
     if (e == cudaSuccess) e = up(lay.items_u, items_u.data(), sizeof(int) * items_u.size());
     if (e == cudaSuccess) e = up(lay.bm2d, bm2d.data(), sizeof(float) * bm2d.size());
@@ -595,6 +597,7 @@ static dos_status solve_impl(dos_ctx *c, int32_t n_iter, float tol, int32_t *h_i
     u.per_oct = c->per_oct;
     u.MP = c->MP; u.chunk = c->chunk; u.n_mat = c->n_mat;
     u.items = (const int *)(c->ws + c->lay.items_u); u.Q = q; u.mat = c->d_mat; u.cdd = a.cdd;
+    for (size_t i = 0; i < sizeof(u.cddc) / sizeof(float); ++i) u.cddc[i] = i < c->h_cdd.size() ? c->h_cdd[i] : 0.f;
     u.bm2d = (const float *)(c->ws + c->lay.bm2d); u.bd2m = (const float *)(c->ws + c->lay.bd2m);
     u.signs = (const unsigned *)(c->ws + c->lay.signs);
     u.fy = a.fy; u.fz = a.fz; u.done = done; u.queue = queue; u.abort_flag = a.abort_flag;

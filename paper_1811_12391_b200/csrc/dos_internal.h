@@ -79,6 +79,7 @@ struct SweepUArgs {
     const uint8_t *mat;      // [Nv]
     const float *sig_t;      // [n_mat] total cross section of this group
     const float *cdd;        // [A][4] cx, cy, cz, cx+cy+cz
+    float cddc[48 * 4];      // the same by value: the cell update reads it from the constant bank, not through the LSU
     const float *bm2d;       // UMMA B operand of the moment-to-discrete: [hi, lo][NAP/8][KP/4][8][4], (angle, lm) = (2l+1) Y_lm, octant 0
     const float *bd2m;       // UMMA B operand of the discrete-to-moment: [hi, lo][NMP/8][A8/4][8][4], (lm, angle) = w Y_lm, octant 0
     const unsigned *signs;   // [8][MP] sign bit of Y_lm(mirror_o Omega) / Y_lm(Omega)

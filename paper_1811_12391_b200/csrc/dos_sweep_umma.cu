@@ -58,8 +58,14 @@ constexpr int WAIT_LIMIT = 1 << 24;     // sleeping polls (>= 64 ns each: second
 #else
 #define TRACE(ev) do { } while (0)
 #endif
+#ifndef DOS_UMMA_CDDC
+#define DOS_UMMA_CDDC 1
+#endif
+#ifndef DOS_UMMA_RCP
+#define DOS_UMMA_RCP 0
+#endif
 #ifndef DOS_UMMA_ABL
-#define DOS_UMMA_ABL 0        // measurement builds only: bit 0 no source-moment copies, 1 no reds, 2 no MMAs, 3 no cell update
+#define DOS_UMMA_ABL 0        // measurement builds only: bit 0 no source-moment copies, 1 no reds, 2 no MMAs, 3 no cell update, 4 no fixup
 #endif
 
 __device__ __forceinline__ int ld_relaxed_gpu(const int *p)
@@ -502,7 +508,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             const uint8_t *mat_col = p.mat + (g.valid ? ((size_t)kg * p.ny + jg) * nx : 0);
             const bool mat4 = (nx & 3) == 0;
             __syncthreads();                          // S2
+#if !DOS_UMMA_CDDC
             const float4 *cdd4 = reinterpret_cast<const float4 *>(s_cdd) + a0;     // (cx, cy, cz, cx+cy+cz) per angle: warp-uniform reads
+#endif
 
             // staging: this lane's pieces of its row of step s, by cp.async; the thread's arrival on the ring slot's
             // mbarrier fires when they have landed
@@ -620,7 +628,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                 if (!r_f) wait_more(&fin_full[fs % RFU], (fs / RFU) & 1, &s_abort, p.abort_flag, 32);
                 TRACE(4);
                 const int fslot = (int)(fs % RFU) * 4 * A;
+#if !DOS_UMMA_RCP
                 const float *rden = s_rden + m0 * A + a0;
+#endif
                 const float sig0 = s_sig[m0];
                 if (t == t_lo) {                      // the lane's first cell: seed the x face with the column's inflow
 #pragma unroll
@@ -677,11 +687,21 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                         float zin = __shfl_up_sync(0xffffffffu, oz[r], DOS_TJ);
                         if (in_y) yin = finy[r * DOS_TK];
                         if (in_z) zin = finz[r * DOS_TJ];
+#if DOS_UMMA_CDDC
+                        const float4 cc = make_float4(p.cddc[(a0 + r) * 4], p.cddc[(a0 + r) * 4 + 1], p.cddc[(a0 + r) * 4 + 2], p.cddc[(a0 + r) * 4 + 3]);
+#else
                         const float4 cc = cdd4[r];
+#endif
                         ix[e] = px[r];
                         yi[e] = yin; zi[e] = zin;
                         const float num = fmaf(cc.x, ix[e], fmaf(cc.y, yin, fmaf(cc.z, zin, qd[e])));
+#if DOS_UMMA_RCP
+                        float rd;                     // 1 / (sigma_t + cx + cy + cz): one MUFU instead of a per-lane table look-up
+                        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rd) : "f"(sig0 + cc.w));
+                        const float c = (DOS_UMMA_ABL & 8) ? 0.f : num * rd;
+#else
                         const float c = (DOS_UMMA_ABL & 8) ? 0.f : num * rden[r];
+#endif
                         pc[e] = c;
                         ox[e] = 2.f * c - ix[e]; oyr[e] = 2.f * c - yin; ozr[e] = 2.f * c - zin;
                         if (fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f) negm |= 1u << e;
@@ -689,12 +709,16 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                     if (!act) negm = 0;
                     // Set-to-zero fixup with rebalance, angle by angle but only for angles some lane of the warp needs it
                     // for: all lanes run the pass in lock-step (a lane with nothing new to pin reproduces its values).
-                    if (__any_sync(0xffffffffu, negm != 0)) {
+                    if (!(DOS_UMMA_ABL & 16) && __any_sync(0xffffffffu, negm != 0)) {
 #pragma unroll
                         for (int e = 0; e < N; ++e) {
                             bool neg = (negm >> e) & 1u;
                             while (__any_sync(0xffffffffu, neg)) {
+#if DOS_UMMA_CDDC
+                                const float4 cc = make_float4(p.cddc[(a0 + C0 + e) * 4], p.cddc[(a0 + C0 + e) * 4 + 1], p.cddc[(a0 + C0 + e) * 4 + 2], 0.f);
+#else
                                 const float4 cc = cdd4[C0 + e];
+#endif
                                 const float gx = ox[e] > 0.f ? 1.f : 0.f, gy = oyr[e] > 0.f ? 1.f : 0.f, gz = ozr[e] > 0.f ? 1.f : 0.f;
                                 const float hx = cc.x * ix[e], hy = cc.y * yi[e], hz = cc.z * zi[e];
                                 const float num = fmaf(fmaf(0.5f, gx, 0.5f), hx, fmaf(fmaf(0.5f, gy, 0.5f), hy, fmaf(fmaf(0.5f, gz, 0.5f), hz, qd[e])));
