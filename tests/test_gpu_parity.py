@@ -70,6 +70,8 @@ VARIANT_CASES = [
     ("config2", dict(nx=5, ny=3, nz=2, voxel=7.0, n_group=3, n_iter=2, sn=2, pl=0)),                # S2/P0: 1 angle, 1 moment
     ("config1", {}),                                                                               # S4/P1, 16^3
     ("config4", dict(nx=18, ny=16, nz=8, voxel=2.0, n_group=3, n_iter=3, n_pos=1, sn=12, pl=4)),   # S12/P4: 21 angles, 25 moments
+    ("config2", dict(nx=19, ny=17, nz=6, voxel=2.2, n_group=2, n_iter=3, sn=10, pl=3)),            # S10/P3: 15 angles (5 x 3 warps)
+    ("config3", dict(nx=17, ny=10, nz=9, voxel=2.5, n_group=2, n_iter=2, sn=14, pl=5)),            # S14/P5: 28 angles (14 x 2 warps)
 ]
 
 
