@@ -148,6 +148,28 @@ dos_status dos_uncollided_sum(dos_ctx *ctx, const dos_source *source, const floa
  * positions given to dos_uncollided_sum since first != 0 -- copied to device [G][nz][ny][nx]. */
 dos_status dos_uncollided_total(dos_ctx *ctx, float *d_phi_u_out);
 
+/* The same ray trace (readings R6-R9) for callers that CANNOT ALLOCATE device memory and so have
+ * no workspace to give dos_create (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no context, no workspace, no cudaMalloc / cudaFree / allocating routine inside. The kernel's scratch
+ * (its [G][n_mat] cross-section table and bad-material flag) lives in a static device array of
+ * DOS_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.
+ *   mesh, source, spectrum   as for dos_create / dos_uncollided (host)
+ *   d_material_ids           device [nz][ny][nx], caller-owned
+ *   sigma_t                  host [n_mat][n_group], > 0; read before the call returns
+ *   d_phi_u_out              device [n_group][nz][ny][nx], caller-owned: the result (bit-identical to dos_uncollided's)
+ *   d_bad_material_out       device, one int32, or NULL: 1 if a material id >= n_mat was met inside the beam (ids are
+ *                            clamped for the table look-up), else 0
+ *   cuda_stream              everything is enqueued on it; nothing is synchronised
+ * LIMIT: n_mat <= 16 and n_group <= 64 (the table must fit the scratch); beyond that DOS_ERR_UNSUPPORTED.
+ * SHARED STATE: every call uses the same array, which keeps the last call's contents; each call rewrites its table and
+ * clears the flag on its stream first. Calls that overlap on the GPU (streams without an ordering between them,
+ * several host threads) RACE; calls on one stream are safe. Errors: message via dos_static_last_error (per thread). */
+#define DOS_STATIC_SCRATCH_BYTES 4352
+dos_status dos_uncollided_static(const dos_mesh *mesh, const uint8_t *d_material_ids, int32_t n_mat, int32_t n_group,
+                                 const float *sigma_t, const dos_source *source, const float *spectrum,
+                                 float *d_phi_u_out, int32_t *d_bad_material_out, void *cuda_stream);
+const char *dos_static_last_error(void);
+
 /* Collided fluence (PAPER.md:39-45 eq. 2-3, :49): for g = 0..G-1, top-down (downscatter only):
  *   Q_fix = first-collision source moments Y_lm(Omega_r) sum_{g'<=g} sigma_sl^{g'->g} phi_u^{g'}
  *           + sum_{g'<g} sigma_sl^{g'->g} phi_c^{g'}[lm]

@@ -9,7 +9,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["dos_api.cu", "dos_kernels.cu", "dos_sweep_umma.cu", "dos_sweep_ffma.cu"]
+SOURCES = ["dos_api.cu", "dos_kernels.cu", "dos_sweep_umma.cu", "dos_sweep_ffma.cu", "dos_static.cu"]
 HEADERS = ["dos_internal.h", "dos_kernels.h", "dos_sm100.cuh", os.path.join("..", "..", "include", "dos.h")]
 LIB = os.path.join(HERE, "libdos.so")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-Xcompiler", "-fPIC"]

@@ -22,7 +22,7 @@ STATUS = {0: "DOS_OK", -1: "DOS_ERR_INVALID_ARG", -2: "DOS_ERR_SHAPE", -3: "DOS_
 
 EXPORTS = ["dos_workspace_bytes", "dos_create", "dos_set_material_host", "dos_uncollided", "dos_uncollided_batch", "dos_uncollided_sum",
            "dos_uncollided_total", "dos_solve", "dos_solve_tol", "dos_set_boundary", "dos_fluence", "dos_dose", "dos_dose_host", "dos_check", "dos_set_option",
-           "dos_profile", "dos_profile_reset", "dos_destroy", "dos_last_error"]
+           "dos_profile", "dos_profile_reset", "dos_destroy", "dos_last_error", "dos_uncollided_static", "dos_static_last_error"]
 
 
 class dos_mesh(C.Structure):
@@ -89,6 +89,11 @@ _lib.dos_destroy.restype = None
 _lib.dos_destroy.argtypes = [C.c_void_p]
 _lib.dos_last_error.restype = C.c_char_p
 _lib.dos_last_error.argtypes = [C.c_void_p]
+_lib.dos_uncollided_static.restype = C.c_int
+_lib.dos_uncollided_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.dos_static_last_error.restype = C.c_char_p
+_lib.dos_static_last_error.argtypes = []
 
 
 class DosError(RuntimeError):
@@ -123,6 +128,22 @@ def _source_struct(s):
     out.tan_half_cone = s["tan_half_cone"]
     out.isotropic = s["isotropic"]
     return out
+
+
+def dos_uncollided_static(mesh, material, sigma_t, source, spectrum, phi_u_out, bad_material_out=None, stream=None):
+    """Ray trace without a context or workspace (include/dos.h: dos_uncollided_static): nothing is allocated; the
+    kernel's scratch is a static device array shared by all calls. material: uint8 device tensor [nz][ny][nx];
+    phi_u_out: float32 device tensor [G][nz][ny][nx]; bad_material_out: int32 device tensor of 1 element or None;
+    stream: a torch.cuda.Stream (default: the current one). Marshalling only."""
+    import torch
+    sig = _f32(sigma_t)
+    n_mat, G = sig.shape
+    m, src, sp = _mesh_struct(mesh), _source_struct(source), _f32(spectrum)
+    st = (stream if stream is not None else torch.cuda.current_stream(material.device)).cuda_stream
+    rc = _lib.dos_uncollided_static(C.byref(m), material.data_ptr(), n_mat, G, sig.ctypes.data, C.byref(src), sp.ctypes.data,
+                                    phi_u_out.data_ptr(), bad_material_out.data_ptr() if bad_material_out is not None else None, st)
+    if rc != DOS_OK:
+        raise DosError(rc, _lib.dos_static_last_error().decode())
 
 
 class _Tables:
