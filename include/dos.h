@@ -215,6 +215,8 @@ dos_status dos_check(dos_ctx *ctx);
  *   "sweep_grid"    number of persistent sweep CTAs
  *   "sweep_angles_per_warp", "sweep_aux_warps", "sweep_angle_split", "sweep_two_per_sm"  shape of the FFMA sweep CTA
  *                   (0 = library default)
+ *   "sweep_ll"      FFMA sweep on small meshes (at most 128 tiles, at most 10 angles per octant): 1 (default) tile faces
+ *                   travel as (value, epoch) pairs that the downwind tile polls directly; 0 the flag protocol of large meshes
  *   "profile"       1: bracket every sweep and ray-trace launch with CUDA events (see dos_profile)  */
 dos_status dos_set_option(dos_ctx *ctx, const char *name, int64_t value);
 

@@ -29,6 +29,8 @@ struct dos_ctx {
     int contraction_pref;                              // 0 auto, 1 FFMA (dos_sweep_ffma.cu), 2 tensor memory (dos_sweep_umma.cu)
     bool umma, umma_ok;                                // the choice in force; the quadrature admits the tensor-memory sweep
     int n_items_u, grid_u;                             // tensor-memory sweep: (quad, tile) items, CTAs
+    int ll_pref;                                       // FFMA sweep: flag-in-data face hand-off on small meshes (1 when the mesh admits it, 0 never)
+    unsigned epoch;                                    // ... its launch counter (never 0)
     int two_per_sm;                                    // FFMA sweep: 64-register two-CTAs-per-SM variant (0 never, 1 from 4 items per SM, 2 always)
     size_t nv;
     cudaStream_t stream;
@@ -101,6 +103,15 @@ static void host_ylm(double mu, double eta, double xi, int L, double *y)
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
+// Meshes on which the FFMA sweep hands tile faces over as (value, epoch) pairs: few tiles (every tile waits on its
+// upwind tile all the way, so the hand-off latency per hop is what the sweep costs) and at most 10 angles per octant
+// (one polling lane per 16-byte piece of a step's inflow).
+static bool ll_mesh(const dos_mesh *m, int per_oct)
+{
+    const int ntj = (m->ny + DOS_TJ - 1) / DOS_TJ, ntk = (m->nz + DOS_TK - 1) / DOS_TK;
+    return 8 * ntj * ntk <= 1024 && 3 * per_oct <= 32;
+}
+
 // Workspace = n_slots "slots" (everything one source position owns: its uncollided fluence, all groups' moments, the
 // sweep's source, face buffers, flags and boundary buffers; slot b starts slot bytes x b further on) followed by what the
 // positions share (work queue and items, material copy, tables, summed-source buffers).
@@ -113,8 +124,10 @@ static Layout make_layout(const dos_mesh *m, int n_mat, int G, int n_leg, int L,
     const int ntj = (m->ny + DOS_TJ - 1) / DOS_TJ, ntk = (m->nz + DOS_TK - 1) / DOS_TK;
     const int KP = (MP + 7) & ~7, A8 = (per + 7) & ~7, NAP = (per + 15) & ~15, NMP = (MP + 15) & ~15;
     // tile-face buffers, one per (octant, tile), indexed by wavefront diagonal
-    const size_t fy = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK;
-    const size_t fz = (size_t)8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TJ;
+    // (small meshes: room for (value, epoch) pairs -- the FFMA sweep's flag-in-data hand-off, dos_internal.h)
+    const size_t pairs = ll_mesh(m, per) ? 2 : 1;
+    const size_t fy = pairs * 8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TK;
+    const size_t fz = pairs * 8 * ntj * ntk * (m->nx + DOS_FACE_PAD) * per * DOS_TJ;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
     // ---- per slot ----
@@ -182,6 +195,13 @@ static dos_status check_inputs(const dos_mesh *mesh, const dos_xs *xs, const dos
 // it, the FFMA sweep below (measured: S8/P3 on 256x256x64 2.9 ms per sweep against 3.7) and as the fallback.
 static cudaError_t configure_sweep(dos_ctx *c)
 {
+    // flag-in-data hand-off: the pair buffers must not hold anything that reads as a current epoch (the workspace is the
+    // caller's memory; the tensor-memory sweep, if it ran on this context, left plain floats there)
+    if (ll_mesh(&c->mesh, c->per_oct))
+        for (int b = 0; b < c->lay.n_slots; ++b) {
+            cudaError_t e = cudaMemsetAsync(c->ws + (size_t)b * c->lay.slot + c->lay.fy, 0, c->lay.done - c->lay.fy, c->stream);
+            if (e != cudaSuccess) return e;
+        }
     const bool ffma_ok = dos_sweep_ffma_angles_per_warp(c->per_oct, c->L, 0) != 0;
     const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok && c->MP >= 28) || !ffma_ok || c->refl != 0;
     if (want_umma) {
@@ -283,6 +303,7 @@ extern "C" dos_status dos_create(dos_ctx **out, const dos_mesh *mesh, const uint
     c->asplit = default_asplit(per, c->n_items);
     c->chunk = 2;
     c->two_per_sm = 1;
+    c->ll_pref = 1; c->epoch = 0;
     c->umma = false;
     c->grid = c->grid_u = 0;
     c->mat_checked = false;
@@ -641,7 +662,12 @@ static dos_status solve_impl(dos_ctx *c, int32_t n_iter, float tol, int32_t *h_i
             ++sweep_no;
             prof_begin(c, 0);
             if (c->umma) CUDA_TRY(c, dos_launch_sweep_umma(u, c->L, c->grid_u, c->stream));
-            else CUDA_TRY(c, dos_launch_sweep_ffma(a, c->L, c->ag, c->grid, c->two_per_sm, c->stream));
+            else {
+                a.ll = (c->ll_pref && ll_mesh(&c->mesh, c->per_oct) && 3 * a.per_oct <= 32) ? 1 : 0;
+                if (++c->epoch == 0 || c->epoch > 0x7fffffffu) c->epoch = 1;
+                a.epoch = (int)c->epoch;
+                CUDA_TRY(c, dos_launch_sweep_ffma(a, c->L, c->ag, c->grid, c->two_per_sm, c->stream));
+            }
             prof_end(c);
             c->launches += 2;
             if (tol >= 0.f) {
@@ -764,6 +790,9 @@ extern "C" dos_status dos_set_option(dos_ctx *c, const char *name, int64_t value
     } else if (!strcmp(name, "sweep_two_per_sm")) {
         if (value < 0 || value > 2) return fail(c, DOS_ERR_INVALID_ARG, "sweep_two_per_sm must be 0, 1 or 2");
         c->two_per_sm = (int)value; reshape = true;
+    } else if (!strcmp(name, "sweep_ll")) {
+        if (value < 0 || value > 1) return fail(c, DOS_ERR_INVALID_ARG, "sweep_ll must be 0 or 1");
+        c->ll_pref = (int)value; reshape = true;      // (re-zeroes the pair buffers)
     } else if (!strcmp(name, "profile")) {
         c->profile = value != 0;
     } else if (!strcmp(name, "sweep_grid")) {

@@ -56,6 +56,12 @@ struct Sweep2Args {
     // behind the pointers above.
     int n_batch;
     size_t slot_stride;
+    // Small meshes: flag-in-data hand-off of the tile faces. Every face value travels as an 8-byte (value, epoch) pair
+    // written with one store; the downwind tile polls the pairs themselves, so a hop costs one L2 round trip instead of
+    // the chain progress word -> release flag -> poll -> acquire -> allowed word -> copy. fy / fz then hold pairs (twice
+    // the bytes), zeroed once; epoch (> 0) differs from launch to launch so that last sweep's pairs read as "not yet".
+    int ll;
+    int epoch;
 };
 
 cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ang_per_warp, int grid, int two_per_sm, cudaStream_t s);

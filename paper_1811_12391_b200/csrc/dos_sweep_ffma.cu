@@ -47,6 +47,18 @@ __device__ __forceinline__ int ld_relaxed(const int *p)
 
 __device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 
+// flag-in-data hand-off (Sweep2Args::ll): one 8-byte store per face value, 16-byte polls of two pairs
+__device__ __forceinline__ void st_pair(float *p, float v, unsigned epoch)
+{
+    asm volatile("st.relaxed.gpu.global.v2.b32 [%0], {%1, %2};" ::"l"(p), "r"(__float_as_uint(v)), "r"(epoch) : "memory");
+}
+__device__ __forceinline__ uint4 ld_pairs(const float *p)
+{
+    uint4 v;
+    asm volatile("ld.relaxed.gpu.global.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+
 // CTA-scope release / acquire on a shared-memory word (service warp <-> compute warps)
 __device__ __forceinline__ void st_release_cta(int *p, int v)
 {
@@ -144,6 +156,7 @@ struct LoadOp {
     const float *src0;
     float *dst0;
     int sstep, dslot, lo, hi, dist, mask;
+    int e0, nval;          // face ops: lane index (kk or jj) of the op's first value, lanes of the upwind tile inside the mesh
 };
 
 struct ItemGeom {
@@ -161,6 +174,7 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
     const int A = p.per_oct, nx = p.nx;
     LoadOp d;
     d.lo = 1; d.hi = 0;                      // empty window
+    d.e0 = 0; d.nval = 0;
     d.src0 = p.Q; d.dst0 = s_q; d.sstep = 0; d.dslot = 0; d.dist = DQ; d.mask = RQ - 1;
     if (op < 32 * MV) {
         const int c = op / MV, v = op - c * MV;
@@ -181,6 +195,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
         if (g.has_y) { d.lo = 0; d.hi = nx + DOS_TK - 2; }
         d.src0 = g.fy_in + a * DOS_TK;
         d.sstep = A * DOS_TK;
+        if (p.ll) { d.src0 = p.fy + 2 * (d.src0 - p.fy); d.sstep *= 2; }      // (value, epoch) pairs
+        d.e0 = 0; d.nval = min(DOS_TK, p.nz - g.tk * DOS_TK);
         d.dst0 = s_fin + a * FINW;
         d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
     } else {
@@ -188,6 +204,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
         if (g.has_z) { d.lo = 0; d.hi = nx + DOS_TJ - 2; }
         d.src0 = g.fz_in + a * DOS_TJ + 4 * h;
         d.sstep = A * DOS_TJ;
+        if (p.ll) { d.src0 = p.fz + 2 * (d.src0 - p.fz); d.sstep *= 2; }
+        d.e0 = 4 * h; d.nval = min(DOS_TJ, p.ny - g.tj * DOS_TJ);
         d.dst0 = s_fin + a * FINW + DOS_TK + 4 * h;
         d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
     }
@@ -284,6 +302,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 s_allowed = (g.has_y || g.has_z) ? -1 : BIG;
             }
             __syncthreads();                          // S2
+            if (p.ll) continue;                       // flag-in-data hand-off: the faces carry their own validity
             int published = 0, spins = 0;
             for (;;) {
                 const int dn = ld_acquire_cta(&s_done);
@@ -360,7 +379,41 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                     for (int f = lane + 32; f < n_fops; f += 32) issue_one(make_op<MP>(32 * MV + f, p, g, s_q, s_fin), tau);
                 cp_async_commit();
             };
-            for (int tau = -DF; tau < 0; ++tau) issue_round(tau);
+            // flag-in-data mode: the pairs of step s are requested one step before they are checked (two 16-byte loads per
+            // lane, kept in registers), checked -- and re-read until every pair the step needs carries this launch's
+            // epoch -- then their values go to the ring slot. A pair is needed if its upwind lane is inside the mesh and
+            // active at that diagonal (the others are never written).
+            const unsigned ep = (unsigned)p.epoch;
+            uint4 ra = make_uint4(0, 0, 0, 0), rb = ra;
+            bool req = false;
+            auto ll_request = [&](int s) {
+                req = op0_on && s >= op0.lo && s <= op0.hi;
+                if (req) {
+                    const float *sp = op0.src0 + (long long)s * op0.sstep;
+                    ra = ld_pairs(sp); rb = ld_pairs(sp + 4);
+                }
+            };
+            auto ll_complete = [&](int s) {
+                if (!req) return;
+                const bool n0 = op0.e0 + 0 < op0.nval && (unsigned)(s - op0.e0 - 0) < (unsigned)nx;
+                const bool n1 = op0.e0 + 1 < op0.nval && (unsigned)(s - op0.e0 - 1) < (unsigned)nx;
+                const bool n2 = op0.e0 + 2 < op0.nval && (unsigned)(s - op0.e0 - 2) < (unsigned)nx;
+                const bool n3 = op0.e0 + 3 < op0.nval && (unsigned)(s - op0.e0 - 3) < (unsigned)nx;
+                const float *sp = op0.src0 + (long long)s * op0.sstep;
+                int spins = 0;
+                while ((n0 && ra.y != ep) || (n1 && ra.w != ep) || (n2 && rb.y != ep) || (n3 && rb.w != ep)) {
+                    if (++spins > DOS_SPIN_LIMIT) { atomicExch(p.abort_flag, 1); break; }      // watchdog, as the service warp's
+                    if ((spins & 255) == 0 && ld_relaxed(p.abort_flag)) break;
+                    ra = ld_pairs(sp); rb = ld_pairs(sp + 4);
+                }
+                *reinterpret_cast<float4 *>(op0.dst0 + (s & op0.mask) * op0.dslot) =
+                    make_float4(__uint_as_float(ra.x), __uint_as_float(ra.z), __uint_as_float(rb.x), __uint_as_float(rb.z));
+            };
+            if (p.ll) {
+                ll_request(0); ll_complete(0); ll_request(1);
+            } else {
+                for (int tau = -DF; tau < 0; ++tau) issue_round(tau);
+            }
             sts_s32(mat_w, mat_of(0, mat_p - 3 * istep));
             sts_s32(mat_w + 128, mat_of(1, mat_p - 2 * istep));
             int reg_m = mat_of(2, mat_p - istep);
@@ -368,7 +421,8 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
             bar_compute(NB);                          // S3: step 0's staged data visible to every warp
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
-                issue_round(t);
+                if (p.ll) { ll_complete(t + 1); ll_request(t + 2); }
+                else issue_round(t);
                 sts_s32(mat_w + ((t + 2) & 3) * 128, reg_m);
                 reg_m = mat_of(t + 3, mat_p);
                 mat_p += istep;
@@ -458,9 +512,11 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
         const bool store_y = valid && jj == DOS_TJ - 1 && g.tj < p.ntj - 1;
         const bool store_z = valid && kk == DOS_TK - 1 && g.tk < p.ntk - 1;
         // running pointers, advanced once per step
-        float *fy_st = p.fy + (size_t)g.id * fstride_y + kk + ((long long)(1 - DOS_TJ) * A + a0) * DOS_TK;
-        float *fz_st = p.fz + (size_t)g.id * fstride_z + jj + ((long long)(1 - DOS_TK) * A + a0) * DOS_TJ;
-        const int fy_inc = A * DOS_TK, fz_inc = A * DOS_TJ;
+        const int lls = p.ll ? 2 : 1;               // floats per face value: (value, epoch) pairs in flag-in-data mode
+        const unsigned ep = (unsigned)p.epoch;
+        float *fy_st = p.fy + ((long long)((size_t)g.id * fstride_y) + kk + ((long long)(1 - DOS_TJ) * A + a0) * DOS_TK) * lls;
+        float *fz_st = p.fz + ((long long)((size_t)g.id * fstride_z) + jj + ((long long)(1 - DOS_TK) * A + a0) * DOS_TJ) * lls;
+        const int fy_inc = A * DOS_TK * lls, fz_inc = A * DOS_TJ * lls;
         const unsigned fin_y = smem_addr(s_fin + a0 * FINW + kk), fin_z = smem_addr(s_fin + a0 * FINW + DOS_TK + jj);
         const unsigned psi_w = smem_addr(s_psi + a0 * 32 + lane);
         const unsigned q_row = smem_addr(s_q + lane * MPS);
@@ -532,8 +588,13 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                     if (fminf(ox, fminf(oyr, ozr)) < 0.f)
                         dd_fixup(pc, ox, oyr, ozr, q[r], lds_f32(sig_a + 4 * m0), ccx[r], ccy[r], ccz[r], ix, yin, zin);
                     px[r] = ox; oy[r] = oyr; oz[r] = ozr;
-                    if (store_y) __stcg(fy_st + r * DOS_TK, oyr);
-                    if (store_z) __stcg(fz_st + r * DOS_TJ, ozr);
+                    if (lls == 2) {
+                        if (store_y) st_pair(fy_st + r * (2 * DOS_TK), oyr, ep);
+                        if (store_z) st_pair(fz_st + r * (2 * DOS_TJ), ozr, ep);
+                    } else {
+                        if (store_y) __stcg(fy_st + r * DOS_TK, oyr);
+                        if (store_z) __stcg(fz_st + r * DOS_TJ, ozr);
+                    }
                 }
                 sts_f32(pso + r * 128, pc);
             }

@@ -56,12 +56,14 @@ def test_small_problem_parity(dos, orc, name, ov):
 
 # Every sweep implementation on every kind of problem, whatever the library's default choice is: the tensor-memory sweep
 # (dos_sweep_umma.cu: tcgen05.mma contractions, bulk copies, mbarrier rings), also with an odd hand-off chunk and few
-# persistent CTAs, and the FFMA sweep (dos_sweep_ffma.cu) with and without its two-CTAs-per-SM variant.
+# persistent CTAs, and the FFMA sweep (dos_sweep_ffma.cu) with and without its two-CTAs-per-SM variant and with either
+# face hand-off (small meshes default to (value, epoch) pairs, large ones to release / acquire flags).
 SWEEP_VARIANTS = [
     ("umma", {"sweep_contraction": 2}),
     ("umma-chunk3-grid5", {"sweep_contraction": 2, "sweep_chunk": 3, "sweep_grid": 5}),
     ("ffma", {"sweep_contraction": 1, "sweep_two_per_sm": 0}),
     ("ffma-2cta", {"sweep_contraction": 1, "sweep_two_per_sm": 2}),
+    ("ffma-flags", {"sweep_contraction": 1, "sweep_ll": 0}),      # the large-mesh hand-off protocol on these small meshes
 ]
 VARIANT_CASES = [
     ("config2", dict(nx=37, ny=21, nz=10, voxel=1.0, n_group=4, n_iter=4)),                        # S8/P3, ragged tiles
