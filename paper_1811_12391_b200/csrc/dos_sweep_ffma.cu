@@ -167,7 +167,7 @@ struct ItemGeom {
 
 // Decode load `op` of the current item: ops [0, 32 MV) fetch 4 moments of lane c's cell, the next A
 // fetch the 4 y-face inflows of angle a, the last 2A the 8 z-face inflows of angle a in two halves.
-template <int MP>
+template <int MP, bool LL>
 __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const ItemGeom &g, float *s_q, float *s_fin)
 {
     constexpr int MV = MP / 4, MPS = mps_of(MP);
@@ -195,7 +195,7 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
         if (g.has_y) { d.lo = 0; d.hi = nx + DOS_TK - 2; }
         d.src0 = g.fy_in + a * DOS_TK;
         d.sstep = A * DOS_TK;
-        if (p.ll) { d.src0 = p.fy + 2 * (d.src0 - p.fy); d.sstep *= 2; }      // (value, epoch) pairs
+        if (LL) { d.src0 = p.fy + 2 * (d.src0 - p.fy); d.sstep *= 2; }      // (value, epoch) pairs
         d.e0 = 0; d.nval = min(DOS_TK, p.nz - g.tk * DOS_TK);
         d.dst0 = s_fin + a * FINW;
         d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
@@ -204,7 +204,7 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
         if (g.has_z) { d.lo = 0; d.hi = nx + DOS_TJ - 2; }
         d.src0 = g.fz_in + a * DOS_TJ + 4 * h;
         d.sstep = A * DOS_TJ;
-        if (p.ll) { d.src0 = p.fz + 2 * (d.src0 - p.fz); d.sstep *= 2; }
+        if (LL) { d.src0 = p.fz + 2 * (d.src0 - p.fz); d.sstep *= 2; }
         d.e0 = 4 * h; d.nval = min(DOS_TJ, p.ny - g.tj * DOS_TJ);
         d.dst0 = s_fin + a * FINW + DOS_TK + 4 * h;
         d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
@@ -219,8 +219,9 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
 //   feeder warp    NW + NX        staging copies of the tile-inflow faces, material ids, step count for the
 //                                 service warp
 //   service warp   NW + NX + 1    global hand-off flags (never joins the per-step barrier)
-// TMAX = CTA size bound for the register budget.
-template <int MP, int AG, int TMAX, int MINB>
+// TMAX = CTA size bound for the register budget. LL = flag-in-data hand-off of the tile faces (Sweep2Args::ll; small
+// meshes): an instance of its own, so that the large-mesh kernels carry none of it.
+template <int MP, int AG, int TMAX, int MINB, bool LL>
 __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
 {
     Sweep2Args p = p0;       // Q, phi, fy, fz, done are re-pointed at the item's problem of the batch
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 s_allowed = (g.has_y || g.has_z) ? -1 : BIG;
             }
             __syncthreads();                          // S2
-            if (p.ll) continue;                       // flag-in-data hand-off: the faces carry their own validity
+            if (LL) continue;                         // flag-in-data hand-off: the faces carry their own validity
             int published = 0, spins = 0;
             for (;;) {
                 const int dn = ld_acquire_cta(&s_done);
@@ -354,7 +355,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
             // traffic is light; the same release from an aux or compute thread would wait for that warp's
             // outstanding red.global / st.global round trips to L2 on every step.
             const int n_fops = 3 * A;
-            const LoadOp op0 = make_op<MP>(32 * MV + (lane < n_fops ? lane : 0), p, g, s_q, s_fin);
+            const LoadOp op0 = make_op<MP, LL>(32 * MV + (lane < n_fops ? lane : 0), p, g, s_q, s_fin);
             const bool op0_on = lane < n_fops, more_ops = n_fops > 32;
             const uint8_t *mat_p = p.mat + cbase + 3 * istep;            // material of step t + 3
             const unsigned mat_w = smem_addr(s_mat + lane);
@@ -376,7 +377,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
             auto issue_round = [&](int tau) {         // round tau fetches the tile-inflow faces of step tau + DF
                 if (op0_on) issue_one(op0, tau);
                 if (more_ops)
-                    for (int f = lane + 32; f < n_fops; f += 32) issue_one(make_op<MP>(32 * MV + f, p, g, s_q, s_fin), tau);
+                    for (int f = lane + 32; f < n_fops; f += 32) issue_one(make_op<MP, LL>(32 * MV + f, p, g, s_q, s_fin), tau);
                 cp_async_commit();
             };
             // flag-in-data mode: the pairs of step s are requested one step before they are checked (two 16-byte loads per
@@ -409,7 +410,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 *reinterpret_cast<float4 *>(op0.dst0 + (s & op0.mask) * op0.dslot) =
                     make_float4(__uint_as_float(ra.x), __uint_as_float(ra.z), __uint_as_float(rb.x), __uint_as_float(rb.z));
             };
-            if (p.ll) {
+            if (LL) {
                 ll_request(0); ll_complete(0); ll_request(1);
             } else {
                 for (int tau = -DF; tau < 0; ++tau) issue_round(tau);
@@ -421,7 +422,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
             bar_compute(NB);                          // S3: step 0's staged data visible to every warp
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
-                if (p.ll) { ll_complete(t + 1); ll_request(t + 2); }
+                if (LL) { ll_complete(t + 1); ll_request(t + 2); }
                 else issue_round(t);
                 sts_s32(mat_w + ((t + 2) & 3) * 128, reg_m);
                 reg_m = mat_of(t + 3, mat_p);
@@ -437,8 +438,8 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
             // ---------------- aux warps: staging, material ids, D2M of the previous step ----------------
             const int xw = warp - NW, xt = tid - NW * 32, NXT = NX * 32;
             const int n_ops = 32 * MV;                                   // Q copies; the feeder warp does the faces
-            const LoadOp op0 = make_op<MP>(xt < n_ops ? xt : 0, p, g, s_q, s_fin);
-            const LoadOp op1 = make_op<MP>(xt + NXT < n_ops ? xt + NXT : 0, p, g, s_q, s_fin);
+            const LoadOp op0 = make_op<MP, LL>(xt < n_ops ? xt : 0, p, g, s_q, s_fin);
+            const LoadOp op1 = make_op<MP, LL>(xt + NXT < n_ops ? xt + NXT : 0, p, g, s_q, s_fin);
             const bool op0_on = xt < n_ops, op1_on = xt + NXT < n_ops, more_ops = n_ops > 2 * NXT;
             float *phi_p = p.phi + (cbase - istep) * MP;                 // moments of the cell of step t - 1
             const int phi_inc = istep * MP;
@@ -453,7 +454,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 if (op0_on) issue_one(op0, tau);
                 if (op1_on) issue_one(op1, tau);
                 if (more_ops)
-                    for (int op = xt + 2 * NXT; op < n_ops; op += NXT) issue_one(make_op<MP>(op, p, g, s_q, s_fin), tau);
+                    for (int op = xt + 2 * NXT; op < n_ops; op += NXT) issue_one(make_op<MP, LL>(op, p, g, s_q, s_fin), tau);
                 cp_async_commit();
             };
             for (int tau = -DQ; tau < 0; ++tau) issue_round(tau);
@@ -512,7 +513,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
         const bool store_y = valid && jj == DOS_TJ - 1 && g.tj < p.ntj - 1;
         const bool store_z = valid && kk == DOS_TK - 1 && g.tk < p.ntk - 1;
         // running pointers, advanced once per step
-        const int lls = p.ll ? 2 : 1;               // floats per face value: (value, epoch) pairs in flag-in-data mode
+        constexpr int lls = LL ? 2 : 1;             // floats per face value: (value, epoch) pairs in flag-in-data mode
         const unsigned ep = (unsigned)p.epoch;
         float *fy_st = p.fy + ((long long)((size_t)g.id * fstride_y) + kk + ((long long)(1 - DOS_TJ) * A + a0) * DOS_TK) * lls;
         float *fz_st = p.fz + ((long long)((size_t)g.id * fstride_z) + jj + ((long long)(1 - DOS_TK) * A + a0) * DOS_TJ) * lls;
@@ -615,38 +616,40 @@ typedef void (*sweep_fn)(const Sweep2Args);
 // CTAs share an SM (MP <= 16 only) -- on meshes with many more work items than SMs the second CTA fills the other's
 // barrier and latency stalls (config 4: measured in DESIGN.md section 6)
 template <int MP, int AG>
-static sweep_fn pick_var(int var)
+static sweep_fn pick_var(int var, bool ll)
 {
-    if (var == 1) return sweep_kernel<MP, AG, 768, 1>;
-    if (var == 2) return MP <= 16 ? sweep_kernel<(MP <= 16 ? MP : 4), AG, 512, 2> : nullptr;
-    return sweep_kernel<MP, AG, 512, 1>;
+    if (ll) return (var == 0 && MP <= 16) ? sweep_kernel<(MP <= 16 ? MP : 4), AG, 512, 1, true> : nullptr;
+    if (var == 1) return sweep_kernel<MP, AG, 768, 1, false>;
+    if (var == 2) return MP <= 16 ? sweep_kernel<(MP <= 16 ? MP : 4), AG, 512, 2, false> : nullptr;
+    return sweep_kernel<MP, AG, 512, 1, false>;
 }
 
 template <int MP>
-static sweep_fn pick_ag(int ag, int var)
+static sweep_fn pick_ag(int ag, int var, bool ll)
 {
     switch (ag) {
-        case 1: return pick_var<MP, 1>(var);
-        case 2: return pick_var<MP, 2>(var);
-        case 3: return pick_var<MP, 3>(var);
-        case 4: return pick_var<MP, 4>(var);
+        case 1: return pick_var<MP, 1>(var, ll);
+        case 2: return pick_var<MP, 2>(var, ll);
+        case 3: return pick_var<MP, 3>(var, ll);
+        case 4: return pick_var<MP, 4>(var, ll);
     }
     return nullptr;
 }
 
 // two_per_sm: 1: variant 2 from 4 work items per SM, 2: whenever there are more items than SMs, 0: never (per context)
-static sweep_fn pick(int L, int ag, int per_oct, int n_aux, int n_items, int two_per_sm)
+// ll: the flag-in-data instance (one CTA per SM, P0..P3, at most 10 angles per CTA), nullptr where there is none
+static sweep_fn pick(int L, int ag, int per_oct, int n_aux, int n_items, int two_per_sm, bool ll = false)
 {
     const int warps = per_oct / ag + n_aux + 2, MP = dos_mpad(L);
     int sms = 148, dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int var = warps > 16 ? 1 : ((two_per_sm && MP <= 16 && (two_per_sm == 2 ? n_items > sms : n_items >= 4 * sms)) ? 2 : 0);
     switch (MP) {
-        case 4: return pick_ag<4>(ag, var);
-        case 12: return pick_ag<12>(ag, var);
-        case 16: return pick_ag<16>(ag, var);
-        case 28: return pick_ag<28>(ag, var);
-        case 36: return pick_ag<36>(ag, var);
+        case 4: return pick_ag<4>(ag, var, ll && 3 * per_oct <= 32);
+        case 12: return pick_ag<12>(ag, var, ll && 3 * per_oct <= 32);
+        case 16: return pick_ag<16>(ag, var, ll && 3 * per_oct <= 32);
+        case 28: return ll ? nullptr : pick_ag<28>(ag, var, false);
+        case 36: return ll ? nullptr : pick_ag<36>(ag, var, false);
     }
     return nullptr;
 }
@@ -692,6 +695,8 @@ cudaError_t dos_sweep_ffma_grid(int L, int ag, int n_aux, int per_oct, int n_mat
     const size_t smem = sweep_smem(L, per_oct, n_mat);
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+    if (sweep_fn fl = pick(L, ag, per_oct, n_aux, n_items, two_per_sm, true))       // same shape, same grid
+        if ((e = cudaFuncSetAttribute(fl, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
     int dev = 0, sms = 0, per_sm = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
@@ -709,6 +714,9 @@ cudaError_t dos_launch_sweep_ffma(const Sweep2Args &a, int L, int ag, int grid, 
 {
     sweep_fn f = pick(L, ag, a.per_oct, a.n_aux, a.n_items, two_per_sm);
     if (!f) return cudaErrorInvalidValue;
+    if (a.ll) {      // the caller's buffers hold pairs and an epoch is set: take the flag-in-data instance where there is one
+        if (sweep_fn fl = pick(L, ag, a.per_oct, a.n_aux, a.n_items, two_per_sm, true)) f = fl;
+    }
     const size_t smem = sweep_smem(L, a.per_oct, a.n_mat);
     f<<<grid, (a.n_warps + a.n_aux + 2) * 32, smem, s>>>(a);
     return cudaGetLastError();
