@@ -458,7 +458,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 cp_async_commit();
             };
             for (int tau = -DQ; tau < 0; ++tau) issue_round(tau);
-            cp_async_wait<DF - 1>();
+            cp_async_wait<DQ - 1>();
             bar_compute(NB);                          // S3: step 0's staged data visible to every warp
 
 #pragma unroll 1
@@ -483,7 +483,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                     }
                 }
                 phi_p += phi_inc;
-                cp_async_wait<DF - 1>();              // step t + 1's staged data complete (this thread's copies)
+                cp_async_wait<DQ - 1>();              // step t + 1's staged data (issued DQ rounds ago) complete; the younger rounds stay in flight
                 bar_compute(NB);                      // B_t: ... and visible to all
             }
             if ((unsigned)(T - 1 - t_lo) < (unsigned)nx) {
