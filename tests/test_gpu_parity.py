@@ -91,6 +91,25 @@ def test_every_sweep_variant_parity(dos, orc, case):
         assert_problem_parity(out, ref, f"{name} [{label}]")
 
 
+def test_ffma_sweep_shape_options_parity(dos, orc):
+    """The FFMA sweep's CTA shape knobs (angles per warp, aux warps, an octant's angles split over two CTAs) with either
+    face hand-off: every combination must give the oracle's result (the angle split doubles the face buffers' tile ids,
+    which the (value, epoch) pair layout has to follow)."""
+    p = _make("config2", nx=37, ny=21, nz=10, voxel=1.0, n_group=3, n_iter=3)
+    ref = orc.run_problem(p)
+    for shape in ({"sweep_angles_per_warp": 2}, {"sweep_aux_warps": 1}, {"sweep_angle_split": 2},
+                  {"sweep_angle_split": 5, "sweep_angles_per_warp": 2}):
+        for ll in (1, 0):
+            ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+            ctx.dos_set_option("sweep_contraction", 1)
+            ctx.dos_set_option("sweep_ll", ll)
+            for k, v in shape.items():
+                ctx.dos_set_option(k, v)
+            out = dos.run_problem(p, ctx=ctx)
+            ctx.close()
+            assert_problem_parity(out, ref, f"config2 small [ffma {shape} ll={ll}]")
+
+
 def test_summed_source_mode_parity(dos, orc):
     """several source positions as ONE source, one solve (dos_uncollided_sum)
     against oracle.run_problem_summed; and the state machine of the mode."""
