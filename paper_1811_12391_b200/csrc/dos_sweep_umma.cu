@@ -64,6 +64,12 @@ constexpr int WAIT_LIMIT = 1 << 24;     // sleeping polls (>= 64 ns each: second
 #ifndef DOS_UMMA_RCP
 #define DOS_UMMA_RCP 0
 #endif
+#ifndef DOS_UMMA_FIX
+#define DOS_UMMA_FIX 0      // fixup passes: 0 angle by angle, 1 the chunk's angles together, 2 together when two or more need one
+#endif
+#ifndef DOS_UMMA_FIXRCP
+#define DOS_UMMA_FIXRCP 1
+#endif
 #ifndef DOS_UMMA_ABL
 #define DOS_UMMA_ABL 0        // measurement builds only: bit 0 no source-moment copies, 1 no reds, 2 no MMAs, 3 no cell update, 4 no fixup
 #endif
@@ -710,27 +716,56 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                     // Set-to-zero fixup with rebalance, angle by angle but only for angles some lane of the warp needs it
                     // for: all lanes run the pass in lock-step (a lane with nothing new to pin reproduces its values).
                     if (!(DOS_UMMA_ABL & 16) && __any_sync(0xffffffffu, negm != 0)) {
+                        auto pass = [&](int e) -> bool {      // one fixup pass of angle e; true if the lane found a new negative outflow
+#if DOS_UMMA_CDDC
+                            const float4 cc = make_float4(p.cddc[(a0 + C0 + e) * 4], p.cddc[(a0 + C0 + e) * 4 + 1], p.cddc[(a0 + C0 + e) * 4 + 2], 0.f);
+#else
+                            const float4 cc = cdd4[C0 + e];
+#endif
+                            const float gx = ox[e] > 0.f ? 1.f : 0.f, gy = oyr[e] > 0.f ? 1.f : 0.f, gz = ozr[e] > 0.f ? 1.f : 0.f;
+                            const float hx = cc.x * ix[e], hy = cc.y * yi[e], hz = cc.z * zi[e];
+                            const float num = fmaf(fmaf(0.5f, gx, 0.5f), hx, fmaf(fmaf(0.5f, gy, 0.5f), hy, fmaf(fmaf(0.5f, gz, 0.5f), hz, qd[e])));
+                            const float den = fmaf(gx, cc.x, fmaf(gy, cc.y, fmaf(gz, cc.z, sig0)));
+#if DOS_UMMA_FIXRCP
+                            float rd;                 // den >= sigma_t > 0 and finite: no range handling needed
+                            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rd) : "f"(den));
+                            const float c = num * rd;
+#else
+                            const float c = __fdividef(num, den);
+#endif
+                            pc[e] = c;
+                            ox[e] = gx * (2.f * c - ix[e]);
+                            oyr[e] = gy * (2.f * c - yi[e]);
+                            ozr[e] = gz * (2.f * c - zi[e]);
+                            return act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
+                        };
+#if DOS_UMMA_FIX == 0
 #pragma unroll
                         for (int e = 0; e < N; ++e) {
                             bool neg = (negm >> e) & 1u;
-                            while (__any_sync(0xffffffffu, neg)) {
-#if DOS_UMMA_CDDC
-                                const float4 cc = make_float4(p.cddc[(a0 + C0 + e) * 4], p.cddc[(a0 + C0 + e) * 4 + 1], p.cddc[(a0 + C0 + e) * 4 + 2], 0.f);
-#else
-                                const float4 cc = cdd4[C0 + e];
-#endif
-                                const float gx = ox[e] > 0.f ? 1.f : 0.f, gy = oyr[e] > 0.f ? 1.f : 0.f, gz = ozr[e] > 0.f ? 1.f : 0.f;
-                                const float hx = cc.x * ix[e], hy = cc.y * yi[e], hz = cc.z * zi[e];
-                                const float num = fmaf(fmaf(0.5f, gx, 0.5f), hx, fmaf(fmaf(0.5f, gy, 0.5f), hy, fmaf(fmaf(0.5f, gz, 0.5f), hz, qd[e])));
-                                const float den = fmaf(gx, cc.x, fmaf(gy, cc.y, fmaf(gz, cc.z, sig0)));
-                                const float c = __fdividef(num, den);
-                                pc[e] = c;
-                                ox[e] = gx * (2.f * c - ix[e]);
-                                oyr[e] = gy * (2.f * c - yi[e]);
-                                ozr[e] = gz * (2.f * c - zi[e]);
-                                neg = act && fminf(ox[e], fminf(oyr[e], ozr[e])) < 0.f;
-                            }
+                            while (__any_sync(0xffffffffu, neg)) neg = pass(e);
                         }
+#else
+                        // angles some lane needs a pass for (warp-uniform); with two or more, the passes of all the chunk's
+                        // angles run together so that their dependent chains overlap; a pass of an angle nobody needs it for
+                        // reproduces its values
+                        const unsigned wm = __reduce_or_sync(0xffffffffu, negm);
+                        if (DOS_UMMA_FIX == 1 || (wm & (wm - 1))) {
+                            bool neg = true;
+                            while (__any_sync(0xffffffffu, neg)) {
+                                neg = false;
+#pragma unroll
+                                for (int e = 0; e < N; ++e) neg |= pass(e);
+                            }
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < N; ++e)
+                                if (wm >> e & 1u) {
+                                    bool neg = true;
+                                    while (__any_sync(0xffffffffu, neg)) neg = pass(e);
+                                }
+                        }
+#endif
                     }
                     // Lanes outside their x range compute on whatever they hold: nothing reads it (their neighbours are
                     // outside too, their rows are skipped by the read-back, their stores are predicated off, and px is
