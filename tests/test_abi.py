@@ -135,6 +135,33 @@ def test_null_context_calls_return_status():
     lib.dos_destroy(None)                                        # no-op
 
 
+def test_static_entry_point_validates_before_touching_cuda():
+    """dos_uncollided_static (no context, no workspace, scratch in a static device array): null arguments and sizes
+    beyond the scratch are refused on the host, with a message, before any CUDA call (so this runs without a GPU)."""
+    import ctypes as C
+    import numpy as np
+    from paper_1811_12391_b200 import dos
+    from paper_1811_12391_b200.inputs import make_problem
+    lib = dos.raw()
+    assert lib.dos_uncollided_static(None, None, 2, 4, None, None, None, None, None, None) == -1
+    p = make_problem("config1")
+    mesh, src = dos._mesh_struct(p["mesh"]), dos._source_struct(p["sources"][0])
+    fake = C.c_void_p(256)                                     # never dereferenced: the size check comes first
+    sig = np.ones((2, 65), np.float32)
+    sp = np.ones(65, np.float32)
+    rc = lib.dos_uncollided_static(C.byref(mesh), fake, 2, 65, sig.ctypes.data, C.byref(src), sp.ctypes.data, fake, None, None)
+    assert rc == -6 and b"exceeds the static scratch" in lib.dos_static_last_error()
+    sig = np.ones((17, 4), np.float32)
+    rc = lib.dos_uncollided_static(C.byref(mesh), fake, 17, 4, sig.ctypes.data, C.byref(src), sp.ctypes.data, fake, None, None)
+    assert rc == -6
+    sig = np.zeros((2, 4), np.float32)                         # sigma_t must be > 0
+    rc = lib.dos_uncollided_static(C.byref(mesh), fake, 2, 4, sig.ctypes.data, C.byref(src), sp.ctypes.data, fake, None, None)
+    assert rc == -1 and b"sigma_t" in lib.dos_static_last_error()
+    # the header states the scratch size the library holds per GPU
+    text = open(os.path.join(ROOT, "include", "dos.h")).read()
+    assert "#define DOS_STATIC_SCRATCH_BYTES 4352" in text
+
+
 def test_paper_shaped_workload_has_the_papers_shape():
     """7 groups with edges 100/75/70/60/45/30/20/10 keV, a 50 x 50 x 12.5 cm box on
     64x64x16 or 256x256x64 voxels, 16 source positions, S6/P0 by default; spectrum normalised per source particle."""
