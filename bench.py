@@ -209,7 +209,11 @@ def run_ours(args):
     job_updates = updates_all if sharded else world * updates_all               # what all ranks together process per step
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
-        n_batch = 2 if summed else max(1, min(args.batch, len(mine)))     # summed-source mode needs the n_batch > 1 buffers
+        # positions swept together: 4 on meshes that fill the GPU by themselves (measured: 8 gains nothing at config 4), 16 on
+        # small ones, where a single position leaves most SMs idle (paper-shaped coarse mesh, 16 positions: 105 ms in
+        # batches of 4, 85 ms in one batch of 16); summed-source mode needs the n_batch > 1 buffers
+        batch = args.batch if args.batch > 0 else (16 if nv <= (1 << 17) else 4)
+        n_batch = 2 if summed else max(1, min(batch, len(mine)))
         ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"],
                           device=dev, stream=stream, n_batch=n_batch)
         dose = ctx.new_field(groups=False)
@@ -388,7 +392,7 @@ def main():
     ap.add_argument("--config", default="config5", choices=sorted(WORKLOADS),
                     help="default: config5, the largest single-GPU workload (BASELINE.json's metric is not quoted on a config)")
     ap.add_argument("--positions", type=int, default=0, help="config4 / paper_*: source positions per step (default 36 / 16)")
-    ap.add_argument("--batch", type=int, default=4, help="source positions swept together (dos_uncollided_batch); 1 = one by one")
+    ap.add_argument("--batch", type=int, default=0, help="source positions swept together (dos_uncollided_batch); 1 = one by one, 0 = by mesh size (16 up to 2^17 voxels, else 4)")
     ap.add_argument("--sn", type=int, default=0, help="quadrature order override (paper_*: S2..S8)")
     ap.add_argument("--pl", type=int, default=None, help="scattering order override (paper_*: P0..P1)")
     ap.add_argument("--scan", default="separate", choices=["separate", "summed"],
