@@ -64,6 +64,7 @@ SWEEP_VARIANTS = [
     ("ffma", {"sweep_contraction": 1, "sweep_two_per_sm": 0}),
     ("ffma-2cta", {"sweep_contraction": 1, "sweep_two_per_sm": 2}),
     ("ffma-flags", {"sweep_contraction": 1, "sweep_ll": 0}),      # the large-mesh hand-off protocol on these small meshes
+    ("ffma-grid3", {"sweep_contraction": 1, "sweep_grid": 3}),    # far fewer persistent CTAs than work items: items wait in the queue
 ]
 VARIANT_CASES = [
     ("config2", dict(nx=37, ny=21, nz=10, voxel=1.0, n_group=4, n_iter=4)),                        # S8/P3, ragged tiles
