@@ -60,14 +60,14 @@ __device__ __forceinline__ uint4 ld_pairs(const float *p)
 }
 
 // CTA-scope release / acquire on a shared-memory word (service warp <-> compute warps)
-__device__ __forceinline__ void st_release_cta(int *p, int v)
+// (by 32-bit shared address, converted once per kernel: a generic-to-shared conversion inside a loop costs a read of a
+// special register, SR_CgaCtaId, every time)
+__device__ __forceinline__ void st_release_cta(unsigned a, int v)
 {
-    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
     asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
 }
-__device__ __forceinline__ int ld_acquire_cta(const int *p)
+__device__ __forceinline__ int ld_acquire_cta(unsigned a)
 {
-    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
     int v;
     asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
     return v;
@@ -96,6 +96,10 @@ __device__ __forceinline__ float4 lds_v4(unsigned a)
 }
 __device__ __forceinline__ void sts_f32(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 __device__ __forceinline__ void sts_s32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts_v4(unsigned a, float4 v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 
 // barrier of the compute warps only (the service warp never joins it)
 __device__ __forceinline__ void bar_compute(int n_threads) { asm volatile("bar.sync 1, %0;" ::"r"(n_threads) : "memory"); }
@@ -114,10 +118,9 @@ __device__ __forceinline__ void red_add_v4(float *p, float4 v)
 
 // 16-byte asynchronous global -> shared copy that bypasses L1 (tile faces are written by other SMs
 // during this launch; an L1 line could be stale)
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+__device__ __forceinline__ void cp_async16(unsigned smem_a, const void *gmem)
 {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_a), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -154,8 +157,8 @@ __device__ __forceinline__ void dd_fixup(float &pc, float &ox, float &oy, float 
 // needs (if s lies inside the window [lo, hi]) from src0 + s * sstep (floats) into ring slot s & mask.
 struct LoadOp {
     const float *src0;
-    float *dst0;
-    int sstep, dslot, lo, hi, dist, mask;
+    unsigned dst0;         // shared-memory byte address of ring slot 0
+    int sstep, dslot, lo, hi, dist, mask;      // dslot: bytes between ring slots
     int e0, nval;          // face ops: lane index (kk or jj) of the op's first value, lanes of the upwind tile inside the mesh
 };
 
@@ -175,7 +178,7 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
     LoadOp d;
     d.lo = 1; d.hi = 0;                      // empty window
     d.e0 = 0; d.nval = 0;
-    d.src0 = p.Q; d.dst0 = s_q; d.sstep = 0; d.dslot = 0; d.dist = DQ; d.mask = RQ - 1;
+    d.src0 = p.Q; d.dst0 = smem_addr(s_q); d.sstep = 0; d.dslot = 0; d.dist = DQ; d.mask = RQ - 1;
     if (op < 32 * MV) {
         const int c = op / MV, v = op - c * MV;
         const int jj = c & (DOS_TJ - 1), kk = c / DOS_TJ, skew = jj + kk;
@@ -188,8 +191,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
             d.src0 = p.Q + (cell0 - (long long)istep * skew) * MP + 4 * v;
             d.lo = skew; d.hi = skew + nx - 1;
         }
-        d.dst0 = s_q + c * MPS + 4 * v;
-        d.dslot = 32 * MPS;
+        d.dst0 = smem_addr(s_q + c * MPS + 4 * v);
+        d.dslot = 32 * MPS * 4;
     } else if (op < 32 * MV + A) {
         const int a = op - 32 * MV;
         if (g.has_y) { d.lo = 0; d.hi = nx + DOS_TK - 2; }
@@ -197,8 +200,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
         d.sstep = A * DOS_TK;
         if (LL) { d.src0 = p.fy + 2 * (d.src0 - p.fy); d.sstep *= 2; }      // (value, epoch) pairs
         d.e0 = 0; d.nval = min(DOS_TK, p.nz - g.tk * DOS_TK);
-        d.dst0 = s_fin + a * FINW;
-        d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
+        d.dst0 = smem_addr(s_fin + a * FINW);
+        d.dslot = A * FINW * 4; d.dist = DF; d.mask = RF - 1;
     } else {
         const int idx = op - 32 * MV - A, a = idx >> 1, h = idx & 1;
         if (g.has_z) { d.lo = 0; d.hi = nx + DOS_TJ - 2; }
@@ -206,8 +209,8 @@ __device__ __forceinline__ LoadOp make_op(int op, const Sweep2Args &p, const Ite
         d.sstep = A * DOS_TJ;
         if (LL) { d.src0 = p.fz + 2 * (d.src0 - p.fz); d.sstep *= 2; }
         d.e0 = 4 * h; d.nval = min(DOS_TJ, p.ny - g.tj * DOS_TJ);
-        d.dst0 = s_fin + a * FINW + DOS_TK + 4 * h;
-        d.dslot = A * FINW; d.dist = DF; d.mask = RF - 1;
+        d.dst0 = smem_addr(s_fin + a * FINW + DOS_TK + 4 * h);
+        d.dslot = A * FINW * 4; d.dist = DF; d.mask = RF - 1;
     }
     return d;
 }
@@ -242,7 +245,13 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
     __shared__ int s_done;        // steps finished by the compute/aux warps (written by one aux thread)
     __shared__ int s_allowed;     // last step whose tile-inflow faces are published upwind (service warp)
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // The thread index is read ONCE, through a volatile asm: left to itself the compiler re-reads the special register
+    // (S2R, ~20 cycles) and re-derives lane / jj / kk wherever a loop uses them instead of holding a register -- measured
+    // with ncu at config 4 (64-register variant): 15 % of all executed instructions came from these two source lines.
+    int tid;
+    asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid));
+    const int lane = tid & 31, warp = tid >> 5;
+    const unsigned a_done = smem_addr(&s_done), a_allowed = smem_addr(&s_allowed);
     const bool tick = warp == NW + NX, service = warp == NW + NX + 1, aux = warp >= NW && warp < NW + NX;
     const int jj = lane & (DOS_TJ - 1), kk = lane / DOS_TJ;
     const int skew = jj + kk;
@@ -306,7 +315,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
             if (LL) continue;                         // flag-in-data hand-off: the faces carry their own validity
             int published = 0, spins = 0;
             for (;;) {
-                const int dn = ld_acquire_cta(&s_done);
+                const int dn = ld_acquire_cta(a_done);
                 if (dn - published >= p.chunk || (dn == T && published < T)) {
                     if (lane == 0) st_release(my_flag, dn);       // steps < dn are complete
                     published = dn;
@@ -319,7 +328,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                         fence_acq_rel_gpu();          // relaxed load + fence = acquire of the upwind release
                         avail_y = vy; avail_z = vz;
                         const int al = min(avail_y >= T ? BIG : avail_y - DOS_TJ, avail_z >= T ? BIG : avail_z - DOS_TK);
-                        if (lane == 0) st_release_cta(&s_allowed, al);
+                        if (lane == 0) st_release_cta(a_allowed, al);
                         spins = 0;
                     } else {
                         // watchdog: a hand-off that never arrives must not hang the GPU; the result is then
@@ -327,7 +336,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                         if (++spins > DOS_SPIN_LIMIT) atomicExch(p.abort_flag, 1);
                         if ((spins & 255) == 0 && ld_relaxed(p.abort_flag)) {
                             avail_y = avail_z = BIG;
-                            if (lane == 0) st_release_cta(&s_allowed, BIG);
+                            if (lane == 0) st_release_cta(a_allowed, BIG);
                         }
                         __nanosleep(DOS_POLL_NS);
                     }
@@ -368,7 +377,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 const int s = tau + DF;
                 if (s >= d.lo && s <= d.hi) {
                     while (allowed_c < s) {           // wait until the upwind tiles have published step s
-                        allowed_c = ld_acquire_cta(&s_allowed);
+                        allowed_c = ld_acquire_cta(a_allowed);
                         if (allowed_c < s) __nanosleep(DOS_POLL_NS);
                     }
                     cp_async16(d.dst0 + (s & d.mask) * d.dslot, d.src0 + (long long)s * d.sstep);
@@ -407,8 +416,8 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                     if ((spins & 255) == 0 && ld_relaxed(p.abort_flag)) break;
                     ra = ld_pairs(sp); rb = ld_pairs(sp + 4);
                 }
-                *reinterpret_cast<float4 *>(op0.dst0 + (s & op0.mask) * op0.dslot) =
-                    make_float4(__uint_as_float(ra.x), __uint_as_float(ra.z), __uint_as_float(rb.x), __uint_as_float(rb.z));
+                sts_v4(op0.dst0 + (s & op0.mask) * op0.dslot,
+                       make_float4(__uint_as_float(ra.x), __uint_as_float(ra.z), __uint_as_float(rb.x), __uint_as_float(rb.z)));
             };
             if (LL) {
                 ll_request(0); ll_complete(0); ll_request(1);
@@ -429,7 +438,7 @@ __global__ void __launch_bounds__(TMAX, MINB) sweep_kernel(const Sweep2Args p0)
                 mat_p += istep;
                 cp_async_wait<DF - 1>();              // step t + 1's faces complete (this thread's copies)
                 bar_compute(NB);                      // B_t: ... visible to all; every face store of step t precedes it
-                if (lane == 0) st_release_cta(&s_done, t + 1);
+                if (lane == 0) st_release_cta(a_done, t + 1);
             }
             continue;
         }
