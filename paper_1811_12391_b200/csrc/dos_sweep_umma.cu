@@ -70,6 +70,15 @@ constexpr int WAIT_LIMIT = 1 << 24;     // sleeping polls (>= 64 ns each: second
 #ifndef DOS_UMMA_FIXRCP
 #define DOS_UMMA_FIXRCP 1
 #endif
+// pauses between polls of the helper warps: a step takes ~3 us at S16 and the issuers have thousands of cycles of slack,
+// while every poll is an issue slot taken from the scheduler's three compute warps (100 / 64 ns: 6.77 ms on the 256x256x64
+// test, 300 / 200 ns: 6.72)
+#ifndef DOS_UMMA_HSLEEP
+#define DOS_UMMA_HSLEEP 300     // ns between polls of the issuer and feeder warps
+#endif
+#ifndef DOS_UMMA_SSLEEP
+#define DOS_UMMA_SSLEEP 200     // ... of the service warp
+#endif
 #ifndef DOS_UMMA_ABL
 #define DOS_UMMA_ABL 0        // measurement builds only: bit 0 no source-moment copies, 1 no reds, 2 no MMAs, 3 no cell update, 4 no fixup
 #endif
@@ -326,10 +335,10 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                             avail_y = avail_z = BIG;
                             if (lane == 0) st_release_cta(&s_allowed, BIG);
                         }
-                        __nanosleep(DOS_POLL_NS);
+                        __nanosleep(DOS_UMMA_SSLEEP);
                     }
                 } else {
-                    __nanosleep(4 * DOS_POLL_NS);
+                    __nanosleep(4 * DOS_UMMA_SSLEEP);
                 }
             }
             gs0 += T;
@@ -363,7 +372,7 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
                         for (int d = 16; d >= 1; d >>= 1) mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, d));
                         if (mn >= s - RFU + 1) break;
                         if (((++spins) & 255) == 0 && *(volatile int *)&s_abort) break;
-                        __nanosleep(100);
+                        __nanosleep(DOS_UMMA_HSLEEP);
                     }
                     while (allowed_c < s) {           // wait until the upwind tiles have published step s
                         allowed_c = ld_acquire_cta(&s_allowed);
@@ -392,9 +401,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
                 TRACE(0);
-                wait_bar(&a_full[gs % ASL], (gs / ASL) & 1, &s_abort, p.abort_flag, 100);
+                wait_bar(&a_full[gs % ASL], (gs / ASL) & 1, &s_abort, p.abort_flag, DOS_UMMA_HSLEEP);
                 TRACE(1);
-                wait_bar(&q_empty[gs % DQS], ((gs / DQS) & 1) ^ 1, &s_abort, p.abort_flag, 100);
+                wait_bar(&q_empty[gs % DQS], ((gs / DQS) & 1) ^ 1, &s_abort, p.abort_flag, DOS_UMMA_HSLEEP);
                 TRACE(2);
                 tc_fence_after();
                 {
@@ -439,9 +448,9 @@ __global__ void __launch_bounds__((4 * NG + 4) * 32, 1) sweep_umma_kernel(const 
             for (int t = 0; t < T; ++t) {
                 const unsigned gs = gs0 + t;
                 TRACE(0);
-                wait_bar(&psi_full[gs % PSL], (gs / PSL) & 1, &s_abort, p.abort_flag, 100);
+                wait_bar(&psi_full[gs % PSL], (gs / PSL) & 1, &s_abort, p.abort_flag, DOS_UMMA_HSLEEP);
                 TRACE(1);
-                wait_bar(&phi_empty[gs % DPS], ((gs / DPS) & 1) ^ 1, &s_abort, p.abort_flag, 100);
+                wait_bar(&phi_empty[gs % DPS], ((gs / DPS) & 1) ^ 1, &s_abort, p.abort_flag, DOS_UMMA_HSLEEP);
                 TRACE(2);
                 tc_fence_after();
                 {
