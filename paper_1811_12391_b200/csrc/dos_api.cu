@@ -6,6 +6,7 @@
 #include "dos_internal.h"
 #include "dos_kernels.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -216,10 +217,24 @@ static cudaError_t configure_sweep(dos_ctx *c)
     int as = c->asplit;
     if (as < 1 || c->per_oct % as) as = 1;
     const int ap = c->per_oct / as;
-    const int ag = dos_sweep_ffma_angles_per_warp(ap, c->L, c->ag_pref);
+    int ag = dos_sweep_ffma_angles_per_warp(ap, c->L, c->ag_pref);
     if (ag == 0 || (c->ag_pref > 0 && ag != c->ag_pref)) return cudaErrorInvalidValue;
-    const int nx = dos_sweep_ffma_aux_warps(ap, c->L, ag, c->aux_pref);
+    int nx = dos_sweep_ffma_aux_warps(ap, c->L, ag, c->aux_pref);
     if (ap / ag + nx + 2 > 24) return cudaErrorInvalidValue;
+    // Meshes with many work items per SM run the 64-register variant, several CTAs per SM (dos_sweep_ffma.cu: pick). A CTA
+    // of at most 10 warps fits three times instead of twice: measured at config 4 (S8/P3, 256x256x64), 2 angles per warp
+    // and 3 aux warps (5 + 3 + 2 warps, 3 CTAs per SM) 2.77 ms per sweep against 2.88 for 1 and 4 (16 warps, 2 CTAs);
+    // 2 and 2: 2.79; 2 and 4 (11 warps, 2 CTAs): 3.24; 2 and 1: 3.37. Only when the caller has not fixed the shape.
+    if (c->ag_pref == 0 && c->aux_pref == 0 && c->two_per_sm && c->MP <= 16 && ap / ag + nx + 2 > 10) {
+        int sms = 148, dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const long items = (long)c->n_items * as;
+        if (items >= 16L * sms)      // (128x128x64, 14 items per SM: 0.89 against 0.85 ms -- the smaller CTAs pay off only on long queues)
+            for (int a2 = ag + 1; a2 <= 4; ++a2) {
+                const int x2 = std::min(c->MP / 4, 3);
+                if (ap % a2 == 0 && ap / a2 + x2 + 2 <= 10 && dos_sweep_ffma_angles_per_warp(ap, c->L, a2) == a2) { ag = a2; nx = x2; break; }
+            }
+    }
     int grid = 0;
     cudaError_t e = dos_sweep_ffma_grid(c->L, ag, nx, ap, c->n_mat, c->n_items * as, c->two_per_sm, &grid);
     if (e != cudaSuccess) return e;
