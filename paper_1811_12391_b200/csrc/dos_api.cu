@@ -225,7 +225,8 @@ static cudaError_t configure_sweep(dos_ctx *c)
     // of at most 10 warps fits three times instead of twice: measured at config 4 (S8/P3, 256x256x64), 2 angles per warp
     // and 3 aux warps (5 + 3 + 2 warps, 3 CTAs per SM) 2.77 ms per sweep against 2.88 for 1 and 4 (16 warps, 2 CTAs);
     // 2 and 2: 2.79; 2 and 4 (11 warps, 2 CTAs): 3.24; 2 and 1: 3.37. Only when the caller has not fixed the shape.
-    if (c->ag_pref == 0 && c->aux_pref == 0 && c->two_per_sm && c->MP <= 16 && ap / ag + nx + 2 > 10) {
+    // (paper-shaped fine mesh, S6/P0: 1 angle per warp, 9 warps, 3 CTAs per SM 1.40 ms; 2 per warp, 6 warps, 5 CTAs 1.25; 3: 1.30)
+    if (c->ag_pref == 0 && c->aux_pref == 0 && c->two_per_sm && c->MP <= 16 && ag == 1 && ap / ag + nx + 2 > 6) {
         int sms = 148, dev = 0;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         const long items = (long)c->n_items * as;
