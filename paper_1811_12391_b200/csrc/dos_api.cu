@@ -204,7 +204,7 @@ static cudaError_t configure_sweep(dos_ctx *c)
             if (e != cudaSuccess) return e;
         }
     const bool ffma_ok = dos_sweep_ffma_angles_per_warp(c->per_oct, c->L, 0) != 0;
-    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok && c->MP >= 28) || !ffma_ok || c->refl != 0;
+    const bool want_umma = c->contraction_pref == 2 || (c->contraction_pref == 0 && c->umma_ok && c->MP >= 28 && c->per_oct >= 3) || !ffma_ok || c->refl != 0;
     if (want_umma) {
         if (!c->umma_ok) return cudaErrorInvalidValue;
         int grid = 0;
